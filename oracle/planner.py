@@ -1,0 +1,172 @@
+"""Oracle: FlashCP sharding planner (TEST INFRASTRUCTURE, see oracle/__init__.py).
+
+Follows PAPER.md section 3.1 (problem statement, Eq. 1-3, W_i at PAPER.md:101), section 3.3
+(Whole-Doc / Per-Doc) and Algorithm 1 step by step in the
+deterministic reading listed in DESIGN.md section 3 ("readings of the paper").  Integer arithmetic only.
+
+Notation: documents D=[d_1..d_n] (0-based ``d[k]`` here), CP size N, context
+C = sum d, a shard = (doc, start p, len s, rank j); W = (2p+s+1)*s/2.
+"""
+
+from typing import List, NamedTuple, Sequence
+
+STRATEGY_HYBRID = 0      # Algorithm 1
+STRATEGY_ALL_PER_DOC = 1  # every document Per-Doc
+STRATEGY_WHOLE_DOC = 2   # Whole-Doc only, never Per-Doc
+
+DEFAULT_R_PPM = 1_050_000  # R = 1.05 (paper gives no value; its heuristic reaches 1.04)
+
+
+class Shard(NamedTuple):
+    doc: int
+    start: int   # p_i, tokens of the document preceding the shard
+    len: int     # s_i
+    rank: int    # j with x_ij = 1 (Eq. 1)
+
+
+class Plan(NamedTuple):
+    d: tuple            # document lengths, original packed order
+    n_ranks: int
+    shards: tuple       # canonical: sorted by (rank, doc, start), contiguous neighbours merged
+    per_doc: tuple      # document ids sharded Per-Doc, in the order Algorithm 1 popped them
+    pass_ratios: tuple  # (max_load, sum_load) after each pass of the while loop
+
+
+def W(p: int, s: int) -> int:
+    """Attention workload of a shard with prefix p and length s."""
+    return (2 * p + s + 1) * s // 2
+
+
+def _argmin(keys):
+    best = None
+    for j, key in enumerate(keys):
+        if key is not None and (best is None or key < keys[best]):
+            best = j
+    return best
+
+
+def plan(d: Sequence[int], n_ranks: int, r_ppm: int = DEFAULT_R_PPM,
+         strategy: int = STRATEGY_HYBRID) -> Plan:
+    """Algorithm 1.  Raises ValueError where the C-ABI returns INVALID_ARG."""
+    d = [int(x) for x in d]
+    n, N = len(d), int(n_ranks)
+    if n < 1 or N < 1 or any(x < 1 for x in d) or r_ppm < 1_000_000:
+        raise ValueError("invalid argument")
+    if strategy not in (STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC):
+        raise ValueError("invalid strategy")
+    C = sum(d)
+    if C % N != 0:                       # Eq. 2 needs C/N integral
+        raise ValueError("C not divisible by N")
+    T = C // N
+
+    # line 1: sort D in descending order of length (ties: lower id first)
+    order = sorted(range(n), key=lambda k: (-d[k], k))
+
+    if strategy == STRATEGY_ALL_PER_DOC:
+        k_first, k_last = n, n
+    elif strategy == STRATEGY_WHOLE_DOC:
+        k_first, k_last = 0, 0
+    else:
+        k_first, k_last = 0, n
+
+    pass_ratios = []
+    k_per = k_first
+    while True:                                        # line 4: while Cur_R > R
+        tok = [0] * N
+        load = [0] * N
+        fixed = []                                     # Per-Doc chunk shards (never moved)
+        items = [[] for _ in range(N)]                 # movable Whole-Doc items [doc, start, len]
+        pool = []
+        # Per_Doc_P: 2N chunks, chunks c and 2N-1-c to worker c
+        for i in order[:k_per]:
+            q = d[i] // (2 * N)
+            r = d[i] - 2 * N * q
+            if r > 0:                                   # remainder = head of the document
+                pool.append([i, 0, r])
+            if q > 0:
+                for c in range(2 * N):
+                    j = c if c < N else 2 * N - 1 - c
+                    fixed.append(Shard(i, r + c * q, q, j))
+                    tok[j] += q
+                    load[j] += W(r + c * q, q)
+        for i in order[k_per:]:
+            pool.append([i, 0, d[i]])
+        pool.sort(key=lambda it: (-it[2], it[0]))
+        # lines 5-9: add each document to the least-loaded worker (by workload)
+        for it in pool:
+            j = _argmin([(load[x], x) for x in range(N)])
+            items[j].append(it)
+            tok[j] += it[2]
+            load[j] += W(it[1], it[2])
+        # lines 10-16: make Eq. 2 hold by Whole-Doc sharding
+        while True:
+            a = _argmin([(-tok[x], x) for x in range(N)])   # most tokens, ties lowest rank
+            if tok[a] == T:
+                break
+            e = tok[a] - T
+            while e > 0:
+                b = _argmin([(load[x], x) if tok[x] < T else None for x in range(N)])
+                g = min(e, T - tok[b])
+                fit = [it for it in items[a] if it[2] <= g]
+                if fit:                                  # move a whole item: zero communication
+                    x = min(fit, key=lambda it: (it[2], it[0]))
+                    items[a].remove(x)
+                    moved = x
+                else:                                    # cut the head ("lower segment",
+                    # PAPER.md:124) of the longest item; its tail stays on worker a
+                    x = min(items[a], key=lambda it: (-it[2], it[0]))
+                    moved = [x[0], x[1], g]
+                    x[1] += g
+                    x[2] -= g
+                m = moved[2]
+                w_moved = W(moved[1], m)                 # W(p,s) adds over a cut: W(p,a+b)=W(p,a)+W(p+a,b)
+                load[a] -= w_moved
+                tok[a] -= m
+                items[b].append(moved)
+                load[b] += w_moved
+                tok[b] += m
+                e -= m
+        # line 18: Cur_R = max/avg workload over all CP workers
+        max_load, sum_load = max(load), sum(load)
+        pass_ratios.append((max_load, sum_load))
+        over = max_load * N * 1_000_000 > r_ppm * sum_load
+        if not over or k_per >= k_last:
+            break
+        k_per += 1                                      # lines 19-23: longest doc -> Per-Doc
+
+    shards = list(fixed)
+    for j in range(N):
+        for it in items[j]:
+            shards.append(Shard(it[0], it[1], it[2], j))
+    shards.sort(key=lambda s: (s.rank, s.doc, s.start))
+    merged: List[Shard] = []
+    for s in shards:                                    # merge contiguous neighbours on one rank
+        if merged and merged[-1].rank == s.rank and merged[-1].doc == s.doc \
+                and merged[-1].start + merged[-1].len == s.start:
+            last = merged.pop()
+            merged.append(Shard(s.doc, last.start, last.len + s.len, s.rank))
+        else:
+            merged.append(s)
+    return Plan(tuple(d), N, tuple(merged), tuple(order[:k_per]), tuple(pass_ratios))
+
+
+def rank_tokens(p: Plan) -> List[int]:
+    """Left side of Eq. 2 for every worker."""
+    out = [0] * p.n_ranks
+    for s in p.shards:
+        out[s.rank] += s.len
+    return out
+
+
+def rank_loads(p: Plan) -> List[int]:
+    """Inner sum of Eq. 3 for every worker."""
+    out = [0] * p.n_ranks
+    for s in p.shards:
+        out[s.rank] += W(s.start, s.len)
+    return out
+
+
+def imbalance_ppm(p: Plan) -> int:
+    """floor(1e6 * max_workload / avg_workload)."""
+    loads = rank_loads(p)
+    return max(loads) * p.n_ranks * 1_000_000 // sum(loads)

@@ -1,0 +1,208 @@
+/* fcp.h — C ABI of libfcp: the per-CP-rank hot path of FlashCP (arxiv/paper_2606_08476),
+ * B200 / sm_100a.  plan -> rank layout -> sharding-aware KV gather -> document-masked causal
+ * attention forward/backward -> partial-result (LSE) merge.
+ *
+ * Conventions (section 3.1): documents D=[d_0..d_{n-1}] packed in this order into a
+ * context of C = sum d_k tokens; CP size N ("ranks"); a shard = (doc, start p, len s, rank) =
+ * tokens [p, p+s) of one document; W(p,s) = (2p+s+1)*s/2.
+ *
+ * General rules
+ *  - Every function returns an int: FCP_OK (0) or a negative fcp_status.  Nothing throws or
+ *    aborts across this boundary and there is no global mutable state.
+ *  - "host" pointers are ordinary CPU memory; "device" pointers are CUDA device memory of the
+ *    current device.  The library owns only the opaque host objects it creates (fcp_plan,
+ *    fcp_sched).  It never allocates, frees or synchronises device memory: inputs, outputs
+ *    and workspace are the caller's, every device call is asynchronous on `stream`
+ *    (a cudaStream_t passed as void*; NULL = the legacy default stream).
+ *  - Device tensors are bf16, row-major contiguous, "token-major varlen":
+ *        q, o, dO, dq : [n_q , Hq , D]        k, v, dk, dv : [n_kv, Hkv, D]
+ *        lse          : [Hq, n_q] float32 = natural log of sum_j exp(scale * q.k_j)
+ *    D in {64, 128}; Hq % Hkv == 0; all base pointers 16-byte aligned.
+ */
+#ifndef FCP_H_
+#define FCP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  FCP_OK = 0,
+  FCP_INVALID_ARG = -1,      /* null pointer, n_ranks<1, n_docs<1, d_k<1, C % N != 0, R<1, bad index */
+  FCP_UNSUPPORTED = -2,      /* D not in {64,128}, Hq % Hkv != 0, unknown dtype/strategy */
+  FCP_BUFFER_TOO_SMALL = -3, /* required element count is written to *n_out */
+  FCP_CUDA = -4,             /* a CUDA runtime/driver call or kernel launch failed */
+  FCP_MISALIGNED = -5        /* a device pointer or row pitch is not 16-byte aligned */
+} fcp_status;
+
+const char* fcp_strerror(int status);
+
+/* ------------------------------------------------------------------------------------------
+ * 1. Sharding plan — Algorithm 1, host, integer arithmetic only.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct fcp_plan fcp_plan;               /* opaque, host memory, owned by the library */
+
+typedef struct { int32_t doc, start, len, rank; } fcp_shard;
+
+enum { FCP_STRATEGY_HYBRID = 0,                 /* Algorithm 1: Whole-Doc + Per-Doc */
+       FCP_STRATEGY_ALL_PER_DOC = 1,            /* every document in 2N chunks */
+       FCP_STRATEGY_WHOLE_DOC = 2 };            /* Whole-Doc sharding only */
+
+typedef struct {
+  int64_t imbalance_ppm;   /* target R = max/avg workload times 1e6; >= 1000000;
+                              0 selects the default 1050000 */
+  int32_t strategy;        /* FCP_STRATEGY_* */
+  int32_t reserved;        /* must be 0 */
+} fcp_plan_opts;
+
+/* Builds the plan for documents `doc_lengths[0..n_docs)` (host) on `n_ranks` workers.
+ * Deterministic: fixed tie-breaks.  opts == NULL selects the defaults.
+ * Requires sum(doc_lengths) % n_ranks == 0 (Eq. 2).  *out must be released with
+ * fcp_plan_destroy. */
+int  fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32_t n_ranks,
+                     const fcp_plan_opts* opts, fcp_plan** out);
+void fcp_plan_destroy(fcp_plan* plan);
+
+/* Canonical shard list, sorted by (rank, doc, start), contiguous neighbours merged.
+ * rank == -1 selects all ranks.  Writes min(count, cap) entries to `out` (host, may be NULL when
+ * cap == 0) and the full count to *n_out; returns FCP_BUFFER_TOO_SMALL when count > cap. */
+int  fcp_plan_shards(const fcp_plan* plan, int32_t rank, fcp_shard* out, int32_t cap,
+                     int32_t* n_out);
+/* Ids of the documents Algorithm 1 moved to Per-Doc sharding, in the order they were popped
+ * (descending length).  Same buffer protocol as fcp_plan_shards. */
+int  fcp_plan_perdoc(const fcp_plan* plan, int32_t* doc_ids, int32_t cap, int32_t* n_out);
+
+typedef struct {
+  int32_t  n_ranks, n_docs, n_shards, n_per_doc, n_passes, reserved;
+  int64_t  context_len;          /* C */
+  int64_t  tokens_per_rank;      /* C / N (Eq. 2) */
+  uint64_t max_load, sum_load;   /* max_j and sum_j of sum_i x_ij W_i (Eq. 3) */
+  int64_t  imbalance_ppm;        /* floor(1e6 * max_load * N / sum_load) */
+  int64_t  eq4_tokens;           /* (C/N)(N-1): static full-KV exchange (Eq. 4) */
+  int64_t  eq5_tokens;           /* (N-1) max_j sum_{i in S-hat} x_ij s_i (Eq. 5) */
+  int64_t  max_remote_tokens, sum_remote_tokens;     /* exact KV rows a rank needs from others */
+  int64_t  max_gathered_tokens, sum_gathered_tokens; /* rows of the rank's gathered KV buffer */
+} fcp_stats;
+int  fcp_plan_stats(const fcp_plan* plan, fcp_stats* out);
+
+typedef struct {
+  int32_t  n_shards, n_segs;     /* shards on the rank; documents (KV segments) it has queries of */
+  int64_t  n_q;                  /* local query rows = C/N */
+  int64_t  n_kv;                 /* gathered KV rows = sum_k E_r(k) */
+  int64_t  remote_tokens;        /* gathered rows owned by another rank */
+  int64_t  nonlast_tokens;       /* sum of s_i over the rank's shards in S-hat */
+  uint64_t load;                 /* sum of W_i on the rank */
+} fcp_rank_stats;
+int  fcp_plan_rank_stats(const fcp_plan* plan, int32_t rank, fcp_rank_stats* out);
+
+/* Varlen descriptors of one rank.  All arrays are caller-allocated HOST int32 arrays sized from
+ * fcp_plan_rank_stats (a NULL array is skipped).  Local query rows are the rank's shards in
+ * (doc, start) order; KV segment g holds tokens [0, E_r(k)) of the g-th document (ascending k)
+ * with a query on the rank, E_r(k) = max(p+s) over the rank's shards of k. */
+typedef struct {
+  int32_t* cu_seqlens_q;    /* [n_shards+1] local row offsets of the shards */
+  int32_t* q_pos_off;       /* [n_shards]   p_i: document position of the shard's first query */
+  int32_t* shard_seg;       /* [n_shards]   KV segment the shard reads */
+  int32_t* cu_seqlens_k;    /* [n_segs+1]   row offsets of the segments in the gathered buffer */
+  int32_t* kv_src_start;    /* [n_segs]     global token offset off_k of the segment's document */
+  int32_t* kv_len;          /* [n_segs]     E_r(k) */
+  int32_t* q_token_index;   /* [n_q]        global token of every local query row */
+  int32_t* kv_token_index;  /* [n_kv]       global token of every gathered KV row */
+} fcp_layout;
+int  fcp_rank_layout(const fcp_plan* plan, int32_t rank, fcp_layout* out);
+
+/* ------------------------------------------------------------------------------------------
+ * 2. Sharding-aware KV gather (the "data copy" of PAPER.md:255).
+ *    Copies, for every document k with a query on `rank`, rows [off_k, off_k + E_r(k)) of the
+ *    global K and V [C, Hkv, D] (device) into the contiguous k_out, v_out [n_kv, Hkv, D]
+ *    (device).  One kernel launch.  On one GPU this stands in for "receive + copy": the bytes
+ *    a real CP group would communicate are counted in *counts (host, may be NULL), never sent.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+  int64_t total_tokens, remote_tokens;   /* rows copied; rows owned by another rank */
+  int64_t total_bytes, remote_bytes;     /* K and V together, one pass */
+  int32_t n_ranges, reserved;            /* contiguous source ranges after merging neighbours */
+} fcp_gather_counts;
+int  fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, const void* V,
+                   void* k_out, void* v_out, int32_t n_kv_heads, int32_t head_dim,
+                   void* stream, fcp_gather_counts* counts);
+
+/* ------------------------------------------------------------------------------------------
+ * 3. Tile schedule of one rank: the (shard, q-tile, head) / (segment, kv-tile, kv-head) work
+ *    lists of the attention kernels, ordered by descending cost so that short shards do not
+ *    starve the SMs.  Host object; fcp_sched_upload copies the lists into
+ *    caller-provided device workspace once per (plan, rank).
+ *    Row t of shard i sees keys j of its segment with  j <= q_pos_off[i] + t  and
+ *    j < cu_seqlens_k[g+1]-cu_seqlens_k[g]  (q_pos_off may be negative when the segment is a
+ *    KV *piece* that starts after the document's first token; rows that see no key produce
+ *    o = 0, lse = -inf).
+ * ------------------------------------------------------------------------------------------ */
+typedef struct fcp_sched fcp_sched;             /* opaque, host memory, owned by the library */
+int  fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
+                      const int32_t* shard_seg, int32_t n_shards,
+                      const int32_t* cu_seqlens_k, int32_t n_segs,
+                      int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                      fcp_sched** out);          /* all arrays host */
+int  fcp_sched_from_plan(const fcp_plan* plan, int32_t rank, int32_t n_q_heads,
+                         int32_t n_kv_heads, int32_t head_dim, fcp_sched** out);
+void fcp_sched_destroy(fcp_sched* sched);
+/* Device bytes needed by fcp_sched_upload + fcp_attn_fwd + fcp_attn_bwd (work lists, tile
+ * counters, backward scratch: padded (lse, delta) and the fp32 dq accumulator). */
+int  fcp_sched_workspace_size(const fcp_sched* sched, size_t* device_bytes);
+int  fcp_sched_upload(const fcp_sched* sched, void* workspace, void* stream);
+
+typedef struct {
+  int32_t n_fwd_items, n_bwd_items;   /* work items of the forward / backward kernels */
+  int64_t fwd_kv_tiles;               /* (q-tile, kv-tile) pairs the forward computes, x heads */
+  int64_t bwd_tile_pairs;             /* (kv-tile, q-tile) pairs the backward computes, x heads */
+  uint64_t useful_pairs;              /* sum of unmasked (q,k) pairs over the rank's shards */
+  int64_t n_q, n_kv;
+} fcp_sched_info;
+int  fcp_sched_get_info(const fcp_sched* sched, fcp_sched_info* out);
+
+/* ------------------------------------------------------------------------------------------
+ * 4. Document-masked causal attention, forward and backward.
+ *      forward : o = softmax(scale q K^T + mask) V, lse = log sum exp   (per shard, per head)
+ *      backward: dV = P^T dO, dP = dO V^T, dS = P o (dP - rowsum(dO o O)),
+ *                dQ = scale dS K, dK = scale dS^T Q; dk, dv summed over the G = Hq/Hkv query
+ *                heads of a kv head; they hold only THIS rank's queries' contributions, in the
+ *                layout of k, v (global dK = sum over ranks of scatter-add).
+ *    bf16 tensor-core products with fp32 accumulation, fp32 softmax.
+ * ------------------------------------------------------------------------------------------ */
+typedef struct {
+  const fcp_sched* sched;    /* host */
+  void*       workspace;     /* device, >= fcp_sched_workspace_size bytes, uploaded */
+  const void* q;             /* device bf16 [n_q , Hq , D] */
+  const void* k;             /* device bf16 [n_kv, Hkv, D] */
+  const void* v;             /* device bf16 [n_kv, Hkv, D] */
+  void*       o;             /* device bf16 [n_q , Hq , D]: written by fwd, read by bwd */
+  float*      lse;           /* device f32  [Hq, n_q]    : written by fwd, read by bwd */
+  float       scale;         /* softmax scale, e.g. 1/sqrt(D) */
+  int32_t     reserved;
+  void*       stream;
+} fcp_attn_args;
+int  fcp_attn_fwd(const fcp_attn_args* args);
+int  fcp_attn_bwd(const fcp_attn_args* args, const void* dO, void* dq, void* dk, void* dv);
+
+/* ------------------------------------------------------------------------------------------
+ * 5. Partial-result aggregation: combines attention partials computed over
+ *    two disjoint key sets:  lse = log(e^lse_a + e^lse_b),
+ *    o = e^(lse_a-lse) o_a + e^(lse_b-lse) o_b.  A partial with lse = -inf has weight 0.
+ *    o_* : [n_rows, n_heads, head_dim] (o_dtype: 0 = bf16, 1 = f32), lse_* : [n_heads, n_rows]
+ *    f32.  Outputs may alias the `a` inputs.
+ * ------------------------------------------------------------------------------------------ */
+enum { FCP_DTYPE_BF16 = 0, FCP_DTYPE_F32 = 1 };
+int  fcp_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b,
+               void* o_out, float* lse_out, int64_t n_rows, int32_t n_heads, int32_t head_dim,
+               int32_t o_dtype, void* stream);
+
+/* Library build information: "sm_100a;<git-less version string>". */
+const char* fcp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FCP_H_ */

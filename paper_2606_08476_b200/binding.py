@@ -1,0 +1,319 @@
+"""Thin ctypes binding over libfcp.so (include/fcp.h): argument marshalling only — every step
+of the hot path runs in the library's kernels.  There is no CPU fallback: a missing library
+or a non-zero status raises.  torch is used only for device memory and streams."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfcp.so")
+
+EXPORTS = [
+    "fcp_strerror", "fcp_version", "fcp_plan_create", "fcp_plan_destroy", "fcp_plan_shards",
+    "fcp_plan_perdoc", "fcp_plan_stats", "fcp_plan_rank_stats", "fcp_rank_layout",
+    "fcp_kv_gather", "fcp_sched_create", "fcp_sched_from_plan", "fcp_sched_destroy",
+    "fcp_sched_workspace_size", "fcp_sched_upload", "fcp_sched_get_info", "fcp_attn_fwd",
+    "fcp_attn_bwd", "fcp_merge",
+]
+
+STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC = 0, 1, 2
+
+
+class FcpError(RuntimeError):
+    def __init__(self, status, what):
+        self.status = status
+        super().__init__("%s failed: %s (%d)" % (what, _lib().fcp_strerror(status).decode(), status))
+
+
+class _Shard(C.Structure):
+    _fields_ = [("doc", C.c_int32), ("start", C.c_int32), ("len", C.c_int32), ("rank", C.c_int32)]
+
+
+class _PlanOpts(C.Structure):
+    _fields_ = [("imbalance_ppm", C.c_int64), ("strategy", C.c_int32), ("reserved", C.c_int32)]
+
+
+class _Stats(C.Structure):
+    _fields_ = [("n_ranks", C.c_int32), ("n_docs", C.c_int32), ("n_shards", C.c_int32),
+                ("n_per_doc", C.c_int32), ("n_passes", C.c_int32), ("reserved", C.c_int32),
+                ("context_len", C.c_int64), ("tokens_per_rank", C.c_int64),
+                ("max_load", C.c_uint64), ("sum_load", C.c_uint64), ("imbalance_ppm", C.c_int64),
+                ("eq4_tokens", C.c_int64), ("eq5_tokens", C.c_int64),
+                ("max_remote_tokens", C.c_int64), ("sum_remote_tokens", C.c_int64),
+                ("max_gathered_tokens", C.c_int64), ("sum_gathered_tokens", C.c_int64)]
+
+
+class _RankStats(C.Structure):
+    _fields_ = [("n_shards", C.c_int32), ("n_segs", C.c_int32), ("n_q", C.c_int64),
+                ("n_kv", C.c_int64), ("remote_tokens", C.c_int64), ("nonlast_tokens", C.c_int64),
+                ("load", C.c_uint64)]
+
+
+_I32P = C.POINTER(C.c_int32)
+
+
+class _Layout(C.Structure):
+    _fields_ = [(n, _I32P) for n in ("cu_seqlens_q", "q_pos_off", "shard_seg", "cu_seqlens_k",
+                                     "kv_src_start", "kv_len", "q_token_index", "kv_token_index")]
+
+
+class _GatherCounts(C.Structure):
+    _fields_ = [("total_tokens", C.c_int64), ("remote_tokens", C.c_int64),
+                ("total_bytes", C.c_int64), ("remote_bytes", C.c_int64),
+                ("n_ranges", C.c_int32), ("reserved", C.c_int32)]
+
+
+class _SchedInfo(C.Structure):
+    _fields_ = [("n_fwd_items", C.c_int32), ("n_bwd_items", C.c_int32),
+                ("fwd_kv_tiles", C.c_int64), ("bwd_tile_pairs", C.c_int64),
+                ("useful_pairs", C.c_uint64), ("n_q", C.c_int64), ("n_kv", C.c_int64)]
+
+
+class _AttnArgs(C.Structure):
+    _fields_ = [("sched", C.c_void_p), ("workspace", C.c_void_p), ("q", C.c_void_p),
+                ("k", C.c_void_p), ("v", C.c_void_p), ("o", C.c_void_p), ("lse", C.c_void_p),
+                ("scale", C.c_float), ("reserved", C.c_int32), ("stream", C.c_void_p)]
+
+
+_LIB = None
+
+
+def _lib():
+    global _LIB
+    if _LIB is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libfcp.so is not built: run `python -m paper_2606_08476_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.fcp_strerror.restype = C.c_char_p
+        lib.fcp_strerror.argtypes = [C.c_int]
+        lib.fcp_version.restype = C.c_char_p
+        lib.fcp_plan_destroy.restype = None
+        lib.fcp_plan_destroy.argtypes = [C.c_void_p]
+        lib.fcp_sched_destroy.restype = None
+        lib.fcp_sched_destroy.argtypes = [C.c_void_p]
+        lib.fcp_plan_create.argtypes = [_I32P, C.c_int32, C.c_int32, C.POINTER(_PlanOpts),
+                                        C.POINTER(C.c_void_p)]
+        lib.fcp_plan_shards.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_Shard), C.c_int32, _I32P]
+        lib.fcp_plan_perdoc.argtypes = [C.c_void_p, _I32P, C.c_int32, _I32P]
+        lib.fcp_plan_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
+        lib.fcp_plan_rank_stats.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_RankStats)]
+        lib.fcp_rank_layout.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_Layout)]
+        lib.fcp_kv_gather.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                      C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
+                                      C.POINTER(_GatherCounts)]
+        lib.fcp_sched_create.argtypes = [_I32P, _I32P, _I32P, C.c_int32, _I32P, C.c_int32,
+                                         C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
+        lib.fcp_sched_from_plan.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
+                                            C.POINTER(C.c_void_p)]
+        lib.fcp_sched_workspace_size.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
+        lib.fcp_sched_upload.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.fcp_sched_get_info.argtypes = [C.c_void_p, C.POINTER(_SchedInfo)]
+        lib.fcp_attn_fwd.argtypes = [C.POINTER(_AttnArgs)]
+        lib.fcp_attn_bwd.argtypes = [C.POINTER(_AttnArgs), C.c_void_p, C.c_void_p, C.c_void_p,
+                                     C.c_void_p]
+        lib.fcp_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                  C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_int32,
+                                  C.c_void_p]
+        _LIB = lib
+    return _LIB
+
+
+def _check(status, what):
+    if status != 0:
+        raise FcpError(status, what)
+
+
+def _i32(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+def _p(a):
+    return a.ctypes.data_as(_I32P)
+
+
+def _struct_dict(s):
+    return {n: getattr(s, n) for n, _ in s._fields_ if n != "reserved"}
+
+
+def version():
+    return _lib().fcp_version().decode()
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+class Plan:
+    """fcp_plan: Algorithm 1 sharding plan (host)."""
+
+    def __init__(self, doc_lengths, n_ranks, imbalance_ppm=0, strategy=STRATEGY_HYBRID):
+        d = _i32(doc_lengths)
+        opts = _PlanOpts(int(imbalance_ppm), int(strategy), 0)
+        h = C.c_void_p()
+        _check(_lib().fcp_plan_create(_p(d), d.size, int(n_ranks), C.byref(opts), C.byref(h)),
+               "fcp_plan_create")
+        self._h = h
+        self.n_ranks = int(n_ranks)
+        self.doc_lengths = d.copy()
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            _lib().fcp_plan_destroy(self._h)
+            self._h = None
+
+    def shards(self, rank=-1):
+        """[(doc, start, len, rank)] canonical order."""
+        n = C.c_int32()
+        st = _lib().fcp_plan_shards(self._h, rank, None, 0, C.byref(n))
+        if st not in (0, -3):
+            _check(st, "fcp_plan_shards")
+        buf = (_Shard * max(1, n.value))()
+        _check(_lib().fcp_plan_shards(self._h, rank, buf, n.value, C.byref(n)), "fcp_plan_shards")
+        return [(buf[i].doc, buf[i].start, buf[i].len, buf[i].rank) for i in range(n.value)]
+
+    def per_doc(self):
+        n = C.c_int32()
+        st = _lib().fcp_plan_perdoc(self._h, None, 0, C.byref(n))
+        if st not in (0, -3):
+            _check(st, "fcp_plan_perdoc")
+        buf = np.zeros(max(1, n.value), dtype=np.int32)
+        _check(_lib().fcp_plan_perdoc(self._h, _p(buf), n.value, C.byref(n)), "fcp_plan_perdoc")
+        return [int(x) for x in buf[:n.value]]
+
+    def stats(self):
+        s = _Stats()
+        _check(_lib().fcp_plan_stats(self._h, C.byref(s)), "fcp_plan_stats")
+        return _struct_dict(s)
+
+    def rank_stats(self, rank):
+        s = _RankStats()
+        _check(_lib().fcp_plan_rank_stats(self._h, rank, C.byref(s)), "fcp_plan_rank_stats")
+        return _struct_dict(s)
+
+    def rank_layout(self, rank):
+        """dict of int32 numpy arrays (see fcp_layout in include/fcp.h)."""
+        rs = self.rank_stats(rank)
+        ns, ng = rs["n_shards"], rs["n_segs"]
+        sizes = {"cu_seqlens_q": ns + 1, "q_pos_off": ns, "shard_seg": ns, "cu_seqlens_k": ng + 1,
+                 "kv_src_start": ng, "kv_len": ng, "q_token_index": rs["n_q"],
+                 "kv_token_index": rs["n_kv"]}
+        arrs = {k: np.zeros(max(1, v), dtype=np.int32) for k, v in sizes.items()}
+        lay = _Layout(**{k: _p(a) for k, a in arrs.items()})
+        _check(_lib().fcp_rank_layout(self._h, rank, C.byref(lay)), "fcp_rank_layout")
+        return {k: arrs[k][:sizes[k]] for k in sizes}
+
+    def kv_gather(self, rank, K, V, k_out=None, v_out=None, stream=None):
+        """Device gather of the rank's KV prefixes.  K, V: torch bf16 [C,Hkv,D] on the GPU.
+        Returns (k_out, v_out, counts)."""
+        import torch
+        assert K.is_cuda and V.is_cuda and K.is_contiguous() and V.is_contiguous()
+        Hkv, D = K.shape[1], K.shape[2]
+        n_kv = self.rank_stats(rank)["n_kv"]
+        if k_out is None:
+            k_out = torch.empty((n_kv, Hkv, D), dtype=K.dtype, device=K.device)
+        if v_out is None:
+            v_out = torch.empty((n_kv, Hkv, D), dtype=V.dtype, device=V.device)
+        cnt = _GatherCounts()
+        _check(_lib().fcp_kv_gather(self._h, rank, K.data_ptr(), V.data_ptr(), k_out.data_ptr(),
+                                    v_out.data_ptr(), Hkv, D * K.element_size() // 2,
+                                    _stream_ptr(stream), C.byref(cnt)), "fcp_kv_gather")
+        return k_out, v_out, _struct_dict(cnt)
+
+    def sched(self, rank, n_q_heads, n_kv_heads, head_dim):
+        h = C.c_void_p()
+        _check(_lib().fcp_sched_from_plan(self._h, rank, n_q_heads, n_kv_heads, head_dim,
+                                          C.byref(h)), "fcp_sched_from_plan")
+        return Sched(h, n_q_heads, n_kv_heads, head_dim)
+
+
+class Sched:
+    """fcp_sched: tile schedule of one rank + its device workspace."""
+
+    def __init__(self, handle, n_q_heads, n_kv_heads, head_dim):
+        self._h = handle
+        self.Hq, self.Hkv, self.D = n_q_heads, n_kv_heads, head_dim
+        self.workspace = None
+
+    @classmethod
+    def create(cls, cu_seqlens_q, q_pos_off, shard_seg, cu_seqlens_k, n_q_heads, n_kv_heads,
+               head_dim):
+        cq, pp, sg, ck = _i32(cu_seqlens_q), _i32(q_pos_off), _i32(shard_seg), _i32(cu_seqlens_k)
+        h = C.c_void_p()
+        _check(_lib().fcp_sched_create(_p(cq), _p(pp), _p(sg), pp.size, _p(ck), ck.size - 1,
+                                       n_q_heads, n_kv_heads, head_dim, C.byref(h)),
+               "fcp_sched_create")
+        return cls(h, n_q_heads, n_kv_heads, head_dim)
+
+    def __del__(self):
+        if getattr(self, "_h", None):
+            _lib().fcp_sched_destroy(self._h)
+            self._h = None
+
+    def info(self):
+        s = _SchedInfo()
+        _check(_lib().fcp_sched_get_info(self._h, C.byref(s)), "fcp_sched_get_info")
+        return _struct_dict(s)
+
+    def workspace_size(self):
+        n = C.c_size_t()
+        _check(_lib().fcp_sched_workspace_size(self._h, C.byref(n)), "fcp_sched_workspace_size")
+        return n.value
+
+    def upload(self, device="cuda", stream=None):
+        import torch
+        self.workspace = torch.empty(self.workspace_size(), dtype=torch.uint8, device=device)
+        _check(_lib().fcp_sched_upload(self._h, self.workspace.data_ptr(), _stream_ptr(stream)),
+               "fcp_sched_upload")
+        return self
+
+    def _args(self, q, k, v, o, lse, scale, stream):
+        if self.workspace is None:
+            self.upload(q.device)
+        return _AttnArgs(self._h, self.workspace.data_ptr(), q.data_ptr(), k.data_ptr(),
+                         v.data_ptr(), o.data_ptr(), lse.data_ptr(), float(scale), 0,
+                         _stream_ptr(stream))
+
+    def attn_fwd(self, q, k, v, scale, o=None, lse=None, stream=None):
+        """q [n_q,Hq,D], k,v [n_kv,Hkv,D] torch bf16 on the GPU -> (o bf16, lse f32 [Hq,n_q])."""
+        import torch
+        for t in (q, k, v):
+            assert t.is_cuda and t.is_contiguous() and t.dtype == torch.bfloat16
+        if o is None:
+            o = torch.empty_like(q)
+        if lse is None:
+            lse = torch.empty((self.Hq, q.shape[0]), dtype=torch.float32, device=q.device)
+        a = self._args(q, k, v, o, lse, scale, stream)
+        _check(_lib().fcp_attn_fwd(C.byref(a)), "fcp_attn_fwd")
+        return o, lse
+
+    def attn_bwd(self, q, k, v, o, lse, do, scale, dq=None, dk=None, dv=None, stream=None):
+        import torch
+        for t in (q, k, v, o, do):
+            assert t.is_cuda and t.is_contiguous() and t.dtype == torch.bfloat16
+        dq = torch.empty_like(q) if dq is None else dq
+        dk = torch.empty_like(k) if dk is None else dk
+        dv = torch.empty_like(v) if dv is None else dv
+        a = self._args(q, k, v, o, lse, scale, stream)
+        _check(_lib().fcp_attn_bwd(C.byref(a), do.data_ptr(), dq.data_ptr(), dk.data_ptr(),
+                                   dv.data_ptr()), "fcp_attn_bwd")
+        return dq, dk, dv
+
+
+def merge(o_a, lse_a, o_b, lse_b, o_out=None, lse_out=None, stream=None):
+    """fcp_merge on torch GPU tensors: o_* [rows,H,D] bf16 or f32, lse_* [H,rows] f32."""
+    import torch
+    assert o_a.is_cuda and o_a.is_contiguous() and o_b.is_contiguous()
+    assert o_a.dtype == o_b.dtype and o_a.dtype in (torch.bfloat16, torch.float32)
+    rows, H, D = o_a.shape
+    o_out = torch.empty_like(o_a) if o_out is None else o_out
+    lse_out = torch.empty_like(lse_a) if lse_out is None else lse_out
+    _check(_lib().fcp_merge(o_a.data_ptr(), lse_a.data_ptr(), o_b.data_ptr(), lse_b.data_ptr(),
+                            o_out.data_ptr(), lse_out.data_ptr(), rows, H, D,
+                            0 if o_a.dtype == torch.bfloat16 else 1, _stream_ptr(stream)),
+           "fcp_merge")
+    return o_out, lse_out

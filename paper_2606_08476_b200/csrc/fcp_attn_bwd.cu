@@ -1,0 +1,565 @@
+// Document-masked causal attention backward (formulas in include/fcp.h)
+// for sm_100a.
+//
+// Three launches:
+//   1. fcp_bwd_prep      delta = rowsum(dO o O); (lse*log2e, delta) into a 64-row-padded scratch
+//                        so that every q tile's statistics are one aligned 512-byte bulk copy;
+//                        padding rows get lse = +inf (P = 0: they contribute nothing).
+//   2. fcp_attn_bwd_main one persistent CTA per SM.  A work item is one 128-row KV tile of one
+//                        KV segment for one kv head; it loops over every (shard, 64-row q tile,
+//                        query head of the GQA group) that sees the tile and keeps dK, dV in
+//                        TMEM for the whole item (the GQA sum costs nothing, no atomics):
+//        warp 0     TMA producer  K,V tile once per item; Q, dO, (lse,delta) per iteration
+//        warp 1     MMA issuer    S^T = K Q^T, dP^T = V dO^T (SS);  dV += P^T dO, dK += dS^T Q
+//                                 (A from TMEM);  dQ^T = K^T dS^T (SS, dS^T staged in smem)
+//        warps 4-7  softmax       one KV row per thread: P^T = exp2(S^T c - lse), mask,
+//                                 dS^T = P^T o (dP^T - delta); bf16 P^T/dS^T back into TMEM
+//        warps 8-11 dQ drain      TMEM -> smem (transposed) -> cp.reduce.async.bulk add.f32
+//                                 into the fp32 dq accumulator [Hq][padded rows][D]
+//   3. fcp_bwd_dq_convert dq = bf16(scale * accumulator)
+//
+// TMEM columns: S^T[2] at 0/64 (P^T in cols 0..31, dS^T in cols 32..63 after softmax),
+// dP^T at 128, dQ^T at 192, dV at 256, dK at 384.
+#include <cuda.h>
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include "fcp_internal.h"
+#include "fcp_sm100.cuh"
+#include "fcp_tma.h"
+
+namespace {
+using namespace fcp;
+
+constexpr float kLog2e = 1.4426950408889634f;
+
+// ------------------------------------------------------------------------------------------
+// 1. prepass
+// ------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(256)
+fcp_bwd_prep(const __nv_bfloat16* __restrict__ o, const __nv_bfloat16* __restrict__ dO,
+             const float* __restrict__ lse, const int32_t* __restrict__ tile_meta,
+             float2* __restrict__ lsed, int64_t n_q, int64_t n_q_pad, int Hq) {
+  const int tile = blockIdx.x, head = blockIdx.y;
+  const int row0 = tile_meta[2 * tile], valid = tile_meta[2 * tile + 1];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  constexpr int kPerLane = D / 32;                       // 2 or 4 bf16 per lane
+  for (int r = warp; r < FCP_BQ; r += 8) {
+    float2 out = make_float2(INFINITY, 0.f);
+    if (r < valid) {
+      const int64_t base = ((int64_t)(row0 + r) * Hq + head) * D + lane * kPerLane;
+      float acc = 0.f;
+#pragma unroll
+      for (int i = 0; i < kPerLane; i += 2) {
+        const float2 a = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(o + base + i));
+        const float2 b = __bfloat1622float2(*reinterpret_cast<const __nv_bfloat162*>(dO + base + i));
+        acc += a.x * b.x + a.y * b.y;
+      }
+#pragma unroll
+      for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+      const float l = lse[(int64_t)head * n_q + row0 + r];
+      out = make_float2(l == -INFINITY ? INFINITY : l * kLog2e, acc);
+    }
+    if (lane == 0) lsed[(int64_t)head * n_q_pad + (int64_t)tile * FCP_BQ + r] = out;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// 3. dq convert
+// ------------------------------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(256)
+fcp_bwd_dq_convert(const float* __restrict__ acc, const int32_t* __restrict__ tile_meta,
+                   __nv_bfloat16* __restrict__ dq, int64_t n_q_pad, int Hq, float scale) {
+  const int tile = blockIdx.x, head = blockIdx.y;
+  const int row0 = tile_meta[2 * tile], valid = tile_meta[2 * tile + 1];
+  constexpr int kVecPerRow = D / 8;
+  for (int idx = threadIdx.x; idx < valid * kVecPerRow; idx += blockDim.x) {
+    const int r = idx / kVecPerRow, c = (idx % kVecPerRow) * 8;
+    const float* src = acc + ((int64_t)head * n_q_pad + (int64_t)tile * FCP_BQ + r) * D + c;
+    const float4 a = *reinterpret_cast<const float4*>(src);
+    const float4 b = *reinterpret_cast<const float4*>(src + 4);
+    int4 pk;
+    pk.x = pack_bf16(a.x * scale, a.y * scale);
+    pk.y = pack_bf16(a.z * scale, a.w * scale);
+    pk.z = pack_bf16(b.x * scale, b.y * scale);
+    pk.w = pack_bf16(b.z * scale, b.w * scale);
+    *reinterpret_cast<int4*>(dq + ((int64_t)(row0 + r) * Hq + head) * D + c) = pk;
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// 2. main kernel
+// ------------------------------------------------------------------------------------------
+template <int D>
+struct BwdCfg {
+  static constexpr int kPanels = D / 64;
+  static constexpr int kKVTile = 128 * D * 2;            // K or V tile: kPanels x [128 rows x 128 B]
+  static constexpr int kKVPanel = 128 * 128;
+  static constexpr int kQTile = FCP_BQ * D * 2;          // Q or dO tile: kPanels x [64 rows x 128 B]
+  static constexpr int kQPanel = FCP_BQ * 128;
+  static constexpr int kStat = FCP_BQ * 8;               // (lse, delta) of one q tile
+  static constexpr int kStage = 2 * kQTile + 1024;       // Q, dO, stats (padded)
+  static constexpr int kStages = 2;
+  static constexpr int kDS = 128 * 128;                  // dS^T bf16 [128 kv][64 q]
+  static constexpr int kDQ = FCP_BQ * D * 4;             // dQ staging fp32 [64 q][D]
+  static constexpr int kThreads = 384;
+  static constexpr int kOffKV = 0;
+  static constexpr int kOffStage = 2 * kKVTile;
+  static constexpr int kOffDS = kOffStage + kStages * kStage;
+  static constexpr int kOffDQ = kOffDS + 2 * kDS;
+  static constexpr int kOffBar = kOffDQ + kDQ;
+  static constexpr int kSmemBytes = 1024 + kOffBar + 1024;
+  static constexpr uint32_t kStageTx = 2 * kQTile + kStat;
+  // TMEM columns
+  static constexpr int kColS = 0, kColDP = 128, kColDQ = 192, kColDV = 256, kColDK = 384;
+};
+
+struct BwdBarriers {
+  uint64_t kv_full, kv_free;
+  uint64_t qdo_full[2], qdo_free[2];
+  uint64_t st_full, dpt_free, p_ready;
+  uint64_t ds_free[2];
+  uint64_t dq_full, dq_free;
+  uint64_t dkv_full, dkv_free;
+  uint32_t tmem_base;
+};
+
+__device__ __forceinline__ int snake_item_b(int round, int n_items) {
+  const int g = gridDim.x, b = blockIdx.x;
+  const int idx = round * g + ((round & 1) ? (g - 1 - b) : b);
+  return idx < n_items ? idx : -1;
+}
+
+// Enumerates the inner iterations of an item in the one order every warp role follows:
+// shards seen by the KV tile -> 64-row q tiles -> the G query heads of the kv head.
+struct IterWalk {
+  const BwdSub* subs;
+  int sub, sub_end, qt, n_qt, g, G;
+  BwdSub cur;
+  __device__ IterWalk(const BwdItem& it, const BwdSub* all, int G_)
+      : subs(all), sub(it.sub_begin), sub_end(it.sub_end), qt(0), n_qt(0), g(0), G(G_) {
+    if (sub < sub_end) {
+      cur = subs[sub];
+      n_qt = (cur.q_rows + FCP_BQ - 1) / FCP_BQ;
+    }
+  }
+  __device__ bool done() const { return sub >= sub_end; }
+  __device__ int q_row() const { return cur.q_row0 + qt * FCP_BQ; }
+  __device__ int q_pos() const { return cur.q_pos0 + qt * FCP_BQ; }
+  __device__ int pad_row() const { return cur.pad_row0 + qt * FCP_BQ; }
+  __device__ int valid() const { return min(FCP_BQ, cur.q_rows - qt * FCP_BQ); }
+  __device__ void next() {
+    if (++g < G) return;
+    g = 0;
+    if (++qt < n_qt) return;
+    qt = 0;
+    if (++sub < sub_end) {
+      cur = subs[sub];
+      n_qt = (cur.q_rows + FCP_BQ - 1) / FCP_BQ;
+    }
+  }
+};
+
+__device__ __forceinline__ void bulk_reduce_add_f32(float* gdst, const void* ssrc, uint32_t bytes) {
+  asm volatile(
+      "cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(gdst),
+      "r"(smem_u32(ssrc)), "r"(bytes)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_commit() {
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read0() {
+  asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait0() {
+  asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+template <int D>
+__global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
+fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
+                  const __grid_constant__ CUtensorMap tmap_do,
+                  const __grid_constant__ CUtensorMap tmap_k,
+                  const __grid_constant__ CUtensorMap tmap_v,
+                  const BwdItem* __restrict__ items, int n_items,
+                  const BwdSub* __restrict__ subs, const float2* __restrict__ lsed,
+                  float* __restrict__ dq_acc, __nv_bfloat16* __restrict__ dk,
+                  __nv_bfloat16* __restrict__ dv, int64_t n_q_pad, int Hkv, int G,
+                  float scale, float scale_log2) {
+  using Cfg = BwdCfg<D>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
+                                             ~uintptr_t(1023));
+  uint8_t* k_smem = smem + Cfg::kOffKV;
+  uint8_t* v_smem = k_smem + Cfg::kKVTile;
+  uint8_t* stage_smem = smem + Cfg::kOffStage;
+  uint8_t* ds_smem = smem + Cfg::kOffDS;
+  float* dq_smem = reinterpret_cast<float*>(smem + Cfg::kOffDQ);
+  BwdBarriers* bars = reinterpret_cast<BwdBarriers*>(smem + Cfg::kOffBar);
+
+  const int warp = threadIdx.x >> 5;
+  const int lane = threadIdx.x & 31;
+
+  if (threadIdx.x == 0) {
+    mbar_init(&bars->kv_full, 1);
+    mbar_init(&bars->kv_free, 1);
+    for (int i = 0; i < 2; ++i) {
+      mbar_init(&bars->qdo_full[i], 1);
+      mbar_init(&bars->qdo_free[i], 1);
+      mbar_init(&bars->ds_free[i], 1);
+    }
+    mbar_init(&bars->st_full, 1);
+    mbar_init(&bars->dpt_free, 128);
+    mbar_init(&bars->p_ready, 128);
+    mbar_init(&bars->dq_full, 1);
+    mbar_init(&bars->dq_free, 128);
+    mbar_init(&bars->dkv_full, 1);
+    mbar_init(&bars->dkv_free, 128);
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = bars->tmem_base;
+  const int rounds = (n_items + gridDim.x - 1) / gridDim.x;
+
+  if (warp == 0) {
+    // ------------------------------------------------------------------ TMA producer
+    if (lane == 0) {
+      prefetch_tmap(&tmap_q);
+      prefetch_tmap(&tmap_do);
+      prefetch_tmap(&tmap_k);
+      prefetch_tmap(&tmap_v);
+      uint32_t n = 0, m = 0;          // global iteration / item counters
+      for (int r = 0; r < rounds; ++r) {
+        const int idx = snake_item_b(r, n_items);
+        if (idx < 0) continue;
+        const BwdItem it = items[idx];
+        if (it.n_iters == 0) continue;
+        mbar_wait(&bars->kv_free, (m & 1) ^ 1);
+        mbar_arrive_expect_tx(&bars->kv_full, 2 * Cfg::kKVTile);
+        for (int pn = 0; pn < Cfg::kPanels; ++pn) {
+          tma_load_3d(k_smem + pn * Cfg::kKVPanel, &tmap_k, &bars->kv_full, pn * 64, it.kv_head,
+                      it.kv_row0);
+          tma_load_3d(v_smem + pn * Cfg::kKVPanel, &tmap_v, &bars->kv_full, pn * 64, it.kv_head,
+                      it.kv_row0);
+        }
+        for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
+          const uint32_t st = n % Cfg::kStages;
+          uint8_t* sq = stage_smem + st * Cfg::kStage;
+          const int head = it.kv_head * G + w.g;
+          mbar_wait(&bars->qdo_free[st], ((n / Cfg::kStages) & 1) ^ 1);
+          mbar_arrive_expect_tx(&bars->qdo_full[st], Cfg::kStageTx);
+          for (int pn = 0; pn < Cfg::kPanels; ++pn) {
+            tma_load_3d(sq + pn * Cfg::kQPanel, &tmap_q, &bars->qdo_full[st], pn * 64, head,
+                        w.q_row());
+            tma_load_3d(sq + Cfg::kQTile + pn * Cfg::kQPanel, &tmap_do, &bars->qdo_full[st],
+                        pn * 64, head, w.q_row());
+          }
+          bulk_load_1d(sq + 2 * Cfg::kQTile, lsed + (int64_t)head * n_q_pad + w.pad_row(),
+                       Cfg::kStat, &bars->qdo_full[st]);
+        }
+        ++m;
+      }
+    }
+  } else if (warp == 1) {
+    // ------------------------------------------------------------------ MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc_s = umma_idesc_bf16(128, FCP_BQ, 0, 0);    // S^T, dP^T
+      constexpr uint32_t idesc_kv = umma_idesc_bf16(128, D, 0, 1);        // dV, dK
+      constexpr uint32_t idesc_dq = umma_idesc_bf16(128, FCP_BQ, 1, 1);   // dQ^T
+      const uint32_t k_addr = smem_u32(k_smem), v_addr = smem_u32(v_smem);
+      const uint32_t stage_addr = smem_u32(stage_smem), ds_addr = smem_u32(ds_smem);
+      uint32_t n = 0, m = 0;
+
+      // S^T(n) = K Q^T  or  dP^T(n) = V dO^T : A = kv tile (K-major), B = q/dO tile (K-major)
+      auto issue_kq = [&](uint32_t d_col, uint32_t a_base, uint32_t b_base) {
+#pragma unroll
+        for (int kk = 0; kk < D / 16; ++kk)
+          umma_ss(tmem_base + d_col,
+                  umma_desc_sw128(a_base + (kk >> 2) * Cfg::kKVPanel + (kk & 3) * 32, 16, 1024),
+                  umma_desc_sw128(b_base + (kk >> 2) * Cfg::kQPanel + (kk & 3) * 32, 16, 1024),
+                  idesc_s, kk > 0);
+      };
+
+      for (int r = 0; r < rounds; ++r) {
+        const int idx = snake_item_b(r, n_items);
+        if (idx < 0) continue;
+        const BwdItem it = items[idx];
+        const int I = it.n_iters;
+        if (I == 0) continue;
+        mbar_wait(&bars->kv_full, m & 1);
+        // prologue: S^T and dP^T of the item's first iteration
+        {
+          const uint32_t st = n % Cfg::kStages;
+          mbar_wait(&bars->qdo_full[st], (n / Cfg::kStages) & 1);
+          tc_fence_after();
+          issue_kq(Cfg::kColS + (n & 1) * 64, k_addr, stage_addr + st * Cfg::kStage);
+          mbar_wait(&bars->dpt_free, (n & 1) ^ 1);
+          tc_fence_after();
+          issue_kq(Cfg::kColDP, v_addr, stage_addr + st * Cfg::kStage + Cfg::kQTile);
+          umma_commit(&bars->st_full);
+        }
+        for (int i = 0; i < I; ++i, ++n) {
+          if (i + 1 < I) {                       // next iteration's S^T / dP^T run ahead
+            const uint32_t n1 = n + 1, st1 = n1 % Cfg::kStages;
+            mbar_wait(&bars->qdo_full[st1], (n1 / Cfg::kStages) & 1);
+            tc_fence_after();
+            issue_kq(Cfg::kColS + (n1 & 1) * 64, k_addr, stage_addr + st1 * Cfg::kStage);
+            mbar_wait(&bars->dpt_free, (n1 & 1) ^ 1);      // softmax(n) has read dP^T(n)
+            tc_fence_after();
+            issue_kq(Cfg::kColDP, v_addr, stage_addr + st1 * Cfg::kStage + Cfg::kQTile);
+            umma_commit(&bars->st_full);
+          }
+          const uint32_t st = n % Cfg::kStages;
+          const uint32_t q_base = stage_addr + st * Cfg::kStage, do_base = q_base + Cfg::kQTile;
+          const uint32_t tP = tmem_base + Cfg::kColS + (n & 1) * 64, tDS = tP + 32;
+          mbar_wait(&bars->p_ready, n & 1);
+          if (i == 0) mbar_wait(&bars->dkv_free, (m & 1) ^ 1);
+          mbar_wait(&bars->dq_free, (n & 1) ^ 1);
+          tc_fence_after();
+          // dV += P^T dO, dK += dS^T Q : A from TMEM, B = dO / Q tile as MN-major [K=q][N=D]
+#pragma unroll
+          for (int kk = 0; kk < FCP_BQ / 16; ++kk)
+            umma_ts(tmem_base + Cfg::kColDV, tP + kk * 8,
+                    umma_desc_sw128(do_base + kk * 2048, Cfg::kQPanel, 1024), idesc_kv,
+                    (i > 0 || kk > 0) ? 1u : 0u);
+#pragma unroll
+          for (int kk = 0; kk < FCP_BQ / 16; ++kk)
+            umma_ts(tmem_base + Cfg::kColDK, tDS + kk * 8,
+                    umma_desc_sw128(q_base + kk * 2048, Cfg::kQPanel, 1024), idesc_kv,
+                    (i > 0 || kk > 0) ? 1u : 0u);
+          // dQ^T = K^T dS^T : A = K tile as MN-major [K=kv][M=d], B = dS^T smem MN-major [K=kv][N=q]
+#pragma unroll
+          for (int kk = 0; kk < 128 / 16; ++kk)
+            umma_ss(tmem_base + Cfg::kColDQ,
+                    umma_desc_sw128(k_addr + kk * 2048, Cfg::kKVPanel, 1024),
+                    umma_desc_sw128(ds_addr + (n & 1) * Cfg::kDS + kk * 2048, 1024, 1024),
+                    idesc_dq, kk > 0);
+          umma_commit(&bars->qdo_free[st]);
+          umma_commit(&bars->ds_free[n & 1]);
+          umma_commit(&bars->dq_full);
+        }
+        umma_commit(&bars->dkv_full);
+        umma_commit(&bars->kv_free);
+        ++m;
+      }
+    }
+  } else if (warp >= 4 && warp < 8) {
+    // ------------------------------------------------------------------ softmax / dS
+    const int row = (warp & 3) * 32 + lane;            // KV row of the tile = TMEM lane
+    const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
+    uint32_t n = 0, m = 0;
+    for (int r = 0; r < rounds; ++r) {
+      const int idx = snake_item_b(r, n_items);
+      if (idx < 0) continue;
+      const BwdItem it = items[idx];
+      const bool row_valid = row < it.kv_rows;
+      __nv_bfloat16* dk_row = dk + ((int64_t)(it.kv_row0 + row) * Hkv + it.kv_head) * D;
+      __nv_bfloat16* dv_row = dv + ((int64_t)(it.kv_row0 + row) * Hkv + it.kv_head) * D;
+      if (it.n_iters == 0) {                             // no query sees this tile
+        if (row_valid)
+          for (int c = 0; c < D; c += 8) {
+            *reinterpret_cast<int4*>(dk_row + c) = make_int4(0, 0, 0, 0);
+            *reinterpret_cast<int4*>(dv_row + c) = make_int4(0, 0, 0, 0);
+          }
+        continue;
+      }
+      const int kv_pos = it.kv_pos0 + row;
+      for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
+        const uint32_t st = n % Cfg::kStages;
+        const float2* stat =
+            reinterpret_cast<const float2*>(stage_smem + st * Cfg::kStage + 2 * Cfg::kQTile);
+        const uint32_t tS = tmem_base + lane_addr + Cfg::kColS + (n & 1) * 64;
+        const uint32_t tDP = tmem_base + lane_addr + Cfg::kColDP;
+        uint8_t* ds_row = ds_smem + (n & 1) * Cfg::kDS + row * 128;
+        const int q_pos = w.q_pos();
+        // mask needed when some (kv, q) pair of this warp's rows is invisible
+        const bool need_mask = (it.kv_pos0 + (warp & 3) * 32 + 31 > q_pos) || (it.kv_rows < 128);
+        mbar_wait(&bars->qdo_full[st], (n / Cfg::kStages) & 1);   // (lse, delta) of the q tile landed
+        mbar_wait(&bars->st_full, n & 1);
+        tc_fence_after();
+        uint32_t s[2][32];
+        tmem_ld32(tS, s[0]);
+        tmem_ld32(tS + 32, s[1]);
+        mbar_wait(&bars->ds_free[n & 1], ((n >> 1) & 1) ^ 1);   // dQ^T(n-2) has read dS^T smem
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          uint32_t dp[32];
+          tmem_ld32(tDP + h * 32, dp);
+          tmem_ld_wait();
+          if (h == 1) {
+            tc_fence_before();
+            mbar_arrive(&bars->dpt_free);
+          }
+          uint32_t pk_p[16], pk_ds[16];
+#pragma unroll
+          for (int i = 0; i < 32; i += 2) {
+            const float4 st01 = *reinterpret_cast<const float4*>(stat + h * 32 + i);  // lse0,d0,lse1,d1
+            float p0 = fast_exp2(fmaf(__uint_as_float(s[h][i]), scale_log2, -st01.x));
+            float p1 = fast_exp2(fmaf(__uint_as_float(s[h][i + 1]), scale_log2, -st01.z));
+            if (need_mask) {
+              if (!row_valid || kv_pos > q_pos + h * 32 + i) p0 = 0.f;
+              if (!row_valid || kv_pos > q_pos + h * 32 + i + 1) p1 = 0.f;
+            }
+            const float ds0 = p0 * (__uint_as_float(dp[i]) - st01.y);
+            const float ds1 = p1 * (__uint_as_float(dp[i + 1]) - st01.w);
+            pk_p[i >> 1] = pack_bf16(p0, p1);
+            pk_ds[i >> 1] = pack_bf16(ds0, ds1);
+          }
+          tmem_st16(tS + h * 16, pk_p);
+          tmem_st16(tS + 32 + h * 16, pk_ds);
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {                 // 128-byte swizzled row of dS^T
+            const int chunk = (h * 4 + c) ^ (row & 7);
+            *reinterpret_cast<int4*>(ds_row + chunk * 16) =
+                make_int4(pk_ds[4 * c], pk_ds[4 * c + 1], pk_ds[4 * c + 2], pk_ds[4 * c + 3]);
+          }
+        }
+        fence_proxy_async_smem();
+        tmem_st_wait();
+        tc_fence_before();
+        mbar_arrive(&bars->p_ready);
+      }
+      // item epilogue: dV, dK rows out of TMEM
+      mbar_wait(&bars->dkv_full, m & 1);
+      tc_fence_after();
+#pragma unroll
+      for (int which = 0; which < 2; ++which) {
+        const uint32_t tacc = tmem_base + lane_addr + (which == 0 ? Cfg::kColDV : Cfg::kColDK);
+        const float f = which == 0 ? 1.f : scale;
+        __nv_bfloat16* dst = which == 0 ? dv_row : dk_row;
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c) {
+          uint32_t acc[32];
+          tmem_ld32(tacc + c * 32, acc);
+          tmem_ld_wait();
+          if (row_valid) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              int4 pk;
+              pk.x = pack_bf16(__uint_as_float(acc[8 * i + 0]) * f, __uint_as_float(acc[8 * i + 1]) * f);
+              pk.y = pack_bf16(__uint_as_float(acc[8 * i + 2]) * f, __uint_as_float(acc[8 * i + 3]) * f);
+              pk.z = pack_bf16(__uint_as_float(acc[8 * i + 4]) * f, __uint_as_float(acc[8 * i + 5]) * f);
+              pk.w = pack_bf16(__uint_as_float(acc[8 * i + 6]) * f, __uint_as_float(acc[8 * i + 7]) * f);
+              *reinterpret_cast<int4*>(dst + c * 32 + i * 8) = pk;
+            }
+          }
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(&bars->dkv_free);
+      ++m;
+    }
+  } else if (warp >= 8) {
+    // ------------------------------------------------------------------ dQ drain
+    const int drow = (warp & 3) * 32 + lane;           // d index = TMEM lane of dQ^T
+    const uint32_t tDQ = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + Cfg::kColDQ;
+    const bool leader = threadIdx.x == 8 * 32;
+    uint32_t n = 0;
+    for (int r = 0; r < rounds; ++r) {
+      const int idx = snake_item_b(r, n_items);
+      if (idx < 0) continue;
+      const BwdItem it = items[idx];
+      if (it.n_iters == 0) continue;
+      for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
+        mbar_wait(&bars->dq_full, n & 1);
+        tc_fence_after();
+        uint32_t acc[2][32];
+        tmem_ld32(tDQ, acc[0]);
+        tmem_ld32(tDQ + 32, acc[1]);
+        tmem_ld_wait();
+        tc_fence_before();
+        mbar_arrive(&bars->dq_free);
+        if (leader) bulk_wait_read0();                  // previous reduce has read the staging
+        named_bar_sync(1, 128);
+        if (drow < D) {
+#pragma unroll
+          for (int q = 0; q < FCP_BQ; ++q) dq_smem[q * D + drow] = __uint_as_float(acc[q >> 5][q & 31]);
+        }
+        fence_proxy_async_smem();
+        named_bar_sync(1, 128);
+        if (leader) {
+          const int head = it.kv_head * G + w.g;
+          bulk_reduce_add_f32(dq_acc + ((int64_t)head * n_q_pad + w.pad_row()) * D, dq_smem,
+                              (uint32_t)w.valid() * D * 4);
+          bulk_commit();
+        }
+      }
+    }
+    if (leader) bulk_wait0();
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    __syncwarp();
+    tmem_dealloc<512>(tmem_base);
+  }
+}
+
+template <int D>
+int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void* dq, void* dk,
+               void* dv) {
+  using Cfg = BwdCfg<D>;
+  cudaStream_t st = (cudaStream_t)a->stream;
+  char* ws = static_cast<char*>(a->workspace);
+  const int32_t* tile_meta = reinterpret_cast<const int32_t*>(ws + s->off_shard_meta);
+  float2* lsed = reinterpret_cast<float2*>(ws + s->off_lsed);
+  float* dq_acc = reinterpret_cast<float*>(ws + s->off_dq);
+  const int n_pad_tiles = (int)(s->n_q_pad / FCP_BQ);
+  const size_t dq_bytes = (size_t)s->Hq * s->n_q_pad * D * sizeof(float);
+
+  if (n_pad_tiles > 0) {
+    if (cudaMemsetAsync(dq_acc, 0, dq_bytes, st) != cudaSuccess) return FCP_CUDA;
+    fcp_bwd_prep<D><<<dim3(n_pad_tiles, s->Hq), 256, 0, st>>>(
+        static_cast<const __nv_bfloat16*>(a->o), static_cast<const __nv_bfloat16*>(dO), a->lse,
+        tile_meta, lsed, s->n_q, s->n_q_pad, s->Hq);
+    if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
+  }
+  const int n_items = (int)s->bwd.size();
+  if (n_items > 0) {
+    CUtensorMap mq, mdo, mk, mv;
+    if (!make_tmap_rows(&mq, a->q, D, s->Hq, s->n_q, FCP_BQ) ||
+        !make_tmap_rows(&mdo, dO, D, s->Hq, s->n_q, FCP_BQ) ||
+        !make_tmap_rows(&mk, a->k, D, s->Hkv, s->n_kv, 128) ||
+        !make_tmap_rows(&mv, a->v, D, s->Hkv, s->n_kv, 128))
+      return FCP_CUDA;
+    auto kern = fcp_attn_bwd_main<D>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             Cfg::kSmemBytes) != cudaSuccess)
+      return FCP_CUDA;
+    const int grid = std::min(n_items, num_sms());
+    kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(
+        mq, mdo, mk, mv, reinterpret_cast<const BwdItem*>(ws + s->off_bwd), n_items,
+        reinterpret_cast<const BwdSub*>(ws + s->off_sub), lsed, dq_acc,
+        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), s->n_q_pad, s->Hkv,
+        s->G, a->scale, a->scale * kLog2e);
+    if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
+  }
+  if (n_pad_tiles > 0) {
+    fcp_bwd_dq_convert<D><<<dim3(n_pad_tiles, s->Hq), 256, 0, st>>>(
+        dq_acc, tile_meta, static_cast<__nv_bfloat16*>(dq), s->n_q_pad, s->Hq, a->scale);
+    if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
+  }
+  return FCP_OK;
+}
+
+}  // namespace
+
+extern "C" int fcp_attn_bwd(const fcp_attn_args* a, const void* dO, void* dq, void* dk, void* dv) {
+  if (!a || !a->sched || !a->workspace || !a->q || !a->k || !a->v || !a->o || !a->lse || !dO ||
+      !dq || !dk || !dv)
+    return FCP_INVALID_ARG;
+  const fcp_sched* s = a->sched;
+  for (const void* p : {a->q, a->k, a->v, (const void*)a->o, (const void*)a->workspace, dO,
+                        (const void*)dq, (const void*)dk, (const void*)dv})
+    if (reinterpret_cast<uintptr_t>(p) & 15) return FCP_MISALIGNED;
+  if (s->D == 128) return launch_bwd<128>(a, s, dO, dq, dk, dv);
+  if (s->D == 64) return launch_bwd<64>(a, s, dO, dq, dk, dv);
+  return FCP_UNSUPPORTED;
+}

@@ -1,0 +1,261 @@
+// Memory-bound device entry points of libfcp: sharding-aware KV gather,
+// partial-result merge and the schedule upload.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstring>
+
+#include "fcp_internal.h"
+
+namespace {
+
+// ------------------------------------------------------------------------------------------
+// KV gather: a handful of contiguous row ranges of K and V are copied into k_out / v_out.
+// Everything is expressed in 16-byte chunks.  A CTA copies "slabs" of kSlab chunks; all loads
+// of a thread are issued before its stores (8 x 16 B in flight per thread), loads bypass L1,
+// stores are streaming.  HBM-bound: 2 tensors x (read + write) x rows x Hkv*D*2 bytes.
+// ------------------------------------------------------------------------------------------
+constexpr int kMaxRanges = 120;
+constexpr int kGatherThreads = 256;
+constexpr int kGatherUnroll = 8;
+constexpr int kSlab = kGatherThreads * kGatherUnroll;   // 2048 chunks = 32 KB
+
+struct GatherRanges {
+  int32_t n;
+  int32_t pad;
+  int64_t dst0[kMaxRanges + 1];   // first destination chunk of each range; dst0[n] = total
+  int64_t src0[kMaxRanges];       // first source chunk of each range
+};
+
+__device__ __forceinline__ int4 ld_stream(const int4* p) {
+  int4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v4.s32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ void st_stream(int4* p, const int4& v) {
+  asm volatile("st.global.cs.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y),
+               "r"(v.z), "r"(v.w)
+               : "memory");
+}
+
+__global__ void __launch_bounds__(kGatherThreads)
+fcp_kv_gather_kernel(const int4* __restrict__ K, const int4* __restrict__ V,
+                     int4* __restrict__ k_out, int4* __restrict__ v_out,
+                     const __grid_constant__ GatherRanges rg) {
+  const int64_t total = rg.dst0[rg.n];
+  const int64_t n_slabs = (total + kSlab - 1) / kSlab;
+  for (int64_t slab = blockIdx.x; slab < 2 * n_slabs; slab += gridDim.x) {
+    const bool is_v = slab >= n_slabs;
+    const int64_t c0 = (is_v ? slab - n_slabs : slab) * kSlab;
+    const int4* __restrict__ src = is_v ? V : K;
+    int4* __restrict__ dst = is_v ? v_out : k_out;
+    // range that holds the slab's first chunk (uniform over the CTA)
+    int lo = 0, hi = rg.n - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (rg.dst0[mid] <= c0) lo = mid; else hi = mid - 1;
+    }
+    int4 val[kGatherUnroll];
+    int r = lo;
+#pragma unroll
+    for (int u = 0; u < kGatherUnroll; ++u) {
+      const int64_t c = c0 + u * kGatherThreads + threadIdx.x;
+      if (c < total) {
+        while (c >= rg.dst0[r + 1]) ++r;
+        val[u] = ld_stream(src + rg.src0[r] + (c - rg.dst0[r]));
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kGatherUnroll; ++u) {
+      const int64_t c = c0 + u * kGatherThreads + threadIdx.x;
+      if (c < total) st_stream(dst + c, val[u]);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------
+// Merge: one sub-warp of D/8 lanes per (row, head); the group's first lane computes the two
+// weights from the log-sum-exps and broadcasts them with a warp shuffle.
+// ------------------------------------------------------------------------------------------
+template <typename T> struct Vec8;
+template <> struct Vec8<__nv_bfloat16> {
+  static __device__ void load(const void* base, int64_t idx8, float (&f)[8]) {
+    const int4 raw = reinterpret_cast<const int4*>(base)[idx8];
+    const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&raw);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float2 x = __bfloat1622float2(h[i]);
+      f[2 * i] = x.x;  f[2 * i + 1] = x.y;
+    }
+  }
+  static __device__ void store(void* base, int64_t idx8, const float (&f)[8]) {
+    int4 raw;
+    __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&raw);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(f[2 * i], f[2 * i + 1]);
+    reinterpret_cast<int4*>(base)[idx8] = raw;
+  }
+};
+template <> struct Vec8<float> {
+  static __device__ void load(const void* base, int64_t idx8, float (&f)[8]) {
+    const float4 a = reinterpret_cast<const float4*>(base)[2 * idx8];
+    const float4 b = reinterpret_cast<const float4*>(base)[2 * idx8 + 1];
+    f[0] = a.x; f[1] = a.y; f[2] = a.z; f[3] = a.w; f[4] = b.x; f[5] = b.y; f[6] = b.z; f[7] = b.w;
+  }
+  static __device__ void store(void* base, int64_t idx8, const float (&f)[8]) {
+    reinterpret_cast<float4*>(base)[2 * idx8] = make_float4(f[0], f[1], f[2], f[3]);
+    reinterpret_cast<float4*>(base)[2 * idx8 + 1] = make_float4(f[4], f[5], f[6], f[7]);
+  }
+};
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+fcp_merge_kernel(const void* __restrict__ o_a, const float* __restrict__ lse_a,
+                 const void* __restrict__ o_b, const float* __restrict__ lse_b,
+                 void* o_out, float* lse_out, int64_t n_rows, int n_heads, int head_dim) {
+  const int lanes = head_dim / 8;                       // lanes per (row, head): 8 or 16
+  const int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t pair = gid / lanes;                     // = row * n_heads + head
+  const int sub = (int)(gid % lanes);
+  const bool active = pair < n_rows * n_heads;
+  float wa = 0.f, wb = 0.f;
+  if (active && sub == 0) {
+    const int64_t row = pair / n_heads, head = pair % n_heads;
+    const float la = lse_a[head * n_rows + row], lb = lse_b[head * n_rows + row];
+    const float m = fmaxf(la, lb);
+    float lse = -INFINITY;
+    if (m > -INFINITY) {                                 // guard (-inf) - (-inf)
+      const float ea = __expf(la - m), eb = __expf(lb - m);
+      const float z = ea + eb;
+      wa = ea / z;  wb = eb / z;
+      lse = m + __logf(z);
+    }
+    lse_out[head * n_rows + row] = lse;
+  }
+  const int src_lane = (threadIdx.x & 31) / lanes * lanes;
+  wa = __shfl_sync(0xffffffffu, wa, src_lane);
+  wb = __shfl_sync(0xffffffffu, wb, src_lane);
+  if (!active) return;
+  float a[8], b[8], r[8];
+  Vec8<T>::load(o_a, gid, a);
+  Vec8<T>::load(o_b, gid, b);
+#pragma unroll
+  for (int i = 0; i < 8; ++i) r[i] = wa * a[i] + wb * b[i];
+  Vec8<T>::store(o_out, gid, r);
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+
+}  // namespace
+
+extern "C" int fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, const void* V,
+                             void* k_out, void* v_out, int32_t n_kv_heads, int32_t head_dim,
+                             void* stream, fcp_gather_counts* counts) {
+  if (!plan || rank < 0 || rank >= plan->n_ranks || !K || !V || !k_out || !v_out ||
+      n_kv_heads < 1 || head_dim < 1)
+    return FCP_INVALID_ARG;
+  const int64_t row_bytes = (int64_t)n_kv_heads * head_dim * 2;
+  if (row_bytes % 16 != 0) return FCP_UNSUPPORTED;
+  if (!aligned16(K) || !aligned16(V) || !aligned16(k_out) || !aligned16(v_out))
+    return FCP_MISALIGNED;
+  RankView v;
+  fcp_build_rank_view(*plan, rank, v);
+  // merge ranges that are contiguous in the source (neighbouring documents held whole)
+  std::vector<int64_t> src, len;
+  for (size_t g = 0; g < v.kv_len.size(); ++g) {
+    if (!src.empty() && src.back() + len.back() == v.kv_src_start[g]) {
+      len.back() += v.kv_len[g];
+    } else {
+      src.push_back(v.kv_src_start[g]);
+      len.push_back(v.kv_len[g]);
+    }
+  }
+  if (counts) {
+    counts->total_tokens = v.n_kv;
+    counts->remote_tokens = v.remote;
+    counts->total_bytes = 2 * v.n_kv * row_bytes;
+    counts->remote_bytes = 2 * v.remote * row_bytes;
+    counts->n_ranges = (int32_t)src.size();
+    counts->reserved = 0;
+  }
+  const int64_t cpr = row_bytes / 16;          // chunks per row
+  int num_sms = 148;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return FCP_CUDA;
+  cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+  int64_t dst_row = 0;
+  for (size_t base = 0; base < src.size(); base += kMaxRanges) {
+    GatherRanges rg;
+    std::memset(&rg, 0, sizeof(rg));
+    rg.n = (int32_t)std::min<size_t>(kMaxRanges, src.size() - base);
+    int64_t c = 0;
+    for (int i = 0; i < rg.n; ++i) {
+      rg.dst0[i] = c;
+      rg.src0[i] = src[base + i] * cpr;
+      c += len[base + i] * cpr;
+    }
+    rg.dst0[rg.n] = c;
+    const int64_t slabs = 2 * ((c + kSlab - 1) / kSlab);
+    if (slabs == 0) continue;
+    const int grid = (int)std::min<int64_t>(slabs, (int64_t)num_sms * 8);
+    fcp_kv_gather_kernel<<<grid, kGatherThreads, 0, (cudaStream_t)stream>>>(
+        reinterpret_cast<const int4*>(K), reinterpret_cast<const int4*>(V),
+        reinterpret_cast<int4*>(k_out) + dst_row * cpr, reinterpret_cast<int4*>(v_out) + dst_row * cpr,
+        rg);
+    if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
+    dst_row += c / cpr;
+  }
+  return FCP_OK;
+}
+
+extern "C" int fcp_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b,
+                         void* o_out, float* lse_out, int64_t n_rows, int32_t n_heads,
+                         int32_t head_dim, int32_t o_dtype, void* stream) {
+  if (!o_a || !lse_a || !o_b || !lse_b || !o_out || !lse_out || n_rows < 0 || n_heads < 1)
+    return FCP_INVALID_ARG;
+  if ((head_dim != 64 && head_dim != 128) ||
+      (o_dtype != FCP_DTYPE_BF16 && o_dtype != FCP_DTYPE_F32))
+    return FCP_UNSUPPORTED;
+  if (!aligned16(o_a) || !aligned16(o_b) || !aligned16(o_out)) return FCP_MISALIGNED;
+  if (n_rows == 0) return FCP_OK;
+  const int64_t threads = n_rows * n_heads * (head_dim / 8);
+  const int64_t blocks = (threads + 255) / 256;
+  if (blocks > INT32_MAX) return FCP_INVALID_ARG;
+  if (o_dtype == FCP_DTYPE_BF16)
+    fcp_merge_kernel<__nv_bfloat16><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
+        o_a, lse_a, o_b, lse_b, o_out, lse_out, n_rows, n_heads, head_dim);
+  else
+    fcp_merge_kernel<float><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
+        o_a, lse_a, o_b, lse_b, o_out, lse_out, n_rows, n_heads, head_dim);
+  return cudaGetLastError() == cudaSuccess ? FCP_OK : FCP_CUDA;
+}
+
+extern "C" int fcp_sched_upload(const fcp_sched* s, void* workspace, void* stream) {
+  if (!s || !workspace) return FCP_INVALID_ARG;
+  if (!aligned16(workspace)) return FCP_MISALIGNED;
+  char* w = static_cast<char*>(workspace);
+  cudaStream_t st = (cudaStream_t)stream;
+  auto put = [&](size_t off, const void* src, size_t bytes) {
+    return bytes == 0 ||
+           cudaMemcpyAsync(w + off, src, bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  };
+  std::vector<int32_t> meta;
+  for (size_t i = 0; i + 1 < s->cu_q.size(); ++i) {
+    const int32_t a = s->cu_q[i], len = s->cu_q[i + 1] - a;
+    for (int32_t r0 = 0; r0 < len; r0 += FCP_BQ) {
+      meta.push_back(a + r0);
+      meta.push_back(std::min(FCP_BQ, len - r0));
+    }
+  }
+  bool ok = cudaMemsetAsync(w + s->off_counters, 0, 256, st) == cudaSuccess;
+  ok = ok && put(s->off_fwd, s->fwd.data(), s->fwd.size() * sizeof(FwdItem));
+  ok = ok && put(s->off_bwd, s->bwd.data(), s->bwd.size() * sizeof(BwdItem));
+  ok = ok && put(s->off_sub, s->bwd_sub.data(), s->bwd_sub.size() * sizeof(BwdSub));
+  ok = ok && put(s->off_shard_meta, meta.data(), meta.size() * sizeof(int32_t));
+  // the sources are pageable host vectors that die with this call: wait for the copies
+  ok = ok && cudaStreamSynchronize(st) == cudaSuccess;
+  return ok ? FCP_OK : FCP_CUDA;
+}

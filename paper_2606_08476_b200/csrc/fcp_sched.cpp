@@ -1,0 +1,160 @@
+// Tile schedule of one rank (host part): enumerates the forward (shard, q-tile, head-pack) and
+// backward (segment, kv-tile, kv-head) work items, skips fully masked tiles and orders items by
+// descending cost so that short shards do not starve the SMs (short shards
+// lower kernel efficiency).  The device kernels pull items from these lists with an atomic
+// counter (persistent CTAs).
+#include <algorithm>
+#include <new>
+
+#include "fcp_internal.h"
+
+namespace {
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+}
+
+extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
+                                const int32_t* shard_seg, int32_t n_shards,
+                                const int32_t* cu_seqlens_k, int32_t n_segs, int32_t n_q_heads,
+                                int32_t n_kv_heads, int32_t head_dim, fcp_sched** out) {
+  if (!cu_seqlens_q || !q_pos_off || !shard_seg || !cu_seqlens_k || !out || n_shards < 0 ||
+      n_segs < 0 || n_q_heads < 1 || n_kv_heads < 1)
+    return FCP_INVALID_ARG;
+  if ((head_dim != 64 && head_dim != 128) || n_q_heads % n_kv_heads != 0) return FCP_UNSUPPORTED;
+  if (cu_seqlens_q[0] != 0 || cu_seqlens_k[0] != 0) return FCP_INVALID_ARG;
+  for (int i = 0; i < n_shards; ++i)
+    if (cu_seqlens_q[i + 1] < cu_seqlens_q[i] || shard_seg[i] < 0 || shard_seg[i] >= n_segs)
+      return FCP_INVALID_ARG;
+  for (int g = 0; g < n_segs; ++g)
+    if (cu_seqlens_k[g + 1] < cu_seqlens_k[g]) return FCP_INVALID_ARG;
+
+  fcp_sched* s = new (std::nothrow) fcp_sched();
+  if (!s) return FCP_INVALID_ARG;
+  s->Hq = n_q_heads;  s->Hkv = n_kv_heads;  s->D = head_dim;
+  s->G = n_q_heads / n_kv_heads;
+  s->NQ = (s->G % 2 == 0) ? 2 : 1;
+  s->cu_q.assign(cu_seqlens_q, cu_seqlens_q + n_shards + 1);
+  s->q_pos_off.assign(q_pos_off, q_pos_off + n_shards);
+  s->shard_seg.assign(shard_seg, shard_seg + n_shards);
+  s->cu_k.assign(cu_seqlens_k, cu_seqlens_k + n_segs + 1);
+  s->n_q = s->cu_q.back();
+  s->n_kv = s->cu_k.back();
+
+  // ---- forward items ----
+  const int packs = s->G / s->NQ;
+  s->shard_pad0.resize(n_shards);
+  int64_t pad = 0;
+  for (int i = 0; i < n_shards; ++i) {
+    const int32_t a = s->cu_q[i], len = s->cu_q[i + 1] - a, p = s->q_pos_off[i];
+    const int32_t g = s->shard_seg[i];
+    const int32_t kv0 = s->cu_k[g], kvl = s->cu_k[g + 1] - kv0;
+    s->shard_pad0[i] = (int32_t)pad;
+    pad += (int64_t)(len + FCP_BQ - 1) / FCP_BQ * FCP_BQ;
+    for (int32_t t = 0; t < len; ++t) {          // exact unmasked-pair count (statistic)
+      const int64_t vis = std::min<int64_t>(kvl, (int64_t)p + t + 1);
+      if (vis > 0) s->useful_pairs += (uint64_t)vis;
+    }
+    for (int32_t r0 = 0; r0 < len; r0 += FCP_TQ) {
+      FwdItem it;
+      it.q_row0 = a + r0;
+      it.q_rows = std::min(FCP_TQ, len - r0);
+      it.kv_row0 = kv0;
+      it.kv_len = kvl;
+      it.q_pos0 = p + r0;
+      const int64_t last_vis = std::min<int64_t>(kvl - 1, (int64_t)it.q_pos0 + it.q_rows - 1);
+      it.n_kv_tiles = last_vis < 0 ? 0 : (int32_t)(last_vis / FCP_TK + 1);
+      for (int hk = 0; hk < s->Hkv; ++hk)
+        for (int pk = 0; pk < packs; ++pk) {
+          it.kv_head = hk;
+          it.head0 = hk * s->G + pk * s->NQ;
+          s->fwd.push_back(it);
+          s->fwd_kv_tiles += (int64_t)it.n_kv_tiles * s->NQ;
+        }
+    }
+  }
+  s->n_q_pad = pad;
+  std::stable_sort(s->fwd.begin(), s->fwd.end(),
+                   [](const FwdItem& x, const FwdItem& y) { return x.n_kv_tiles > y.n_kv_tiles; });
+
+  // ---- backward items ----
+  std::vector<std::vector<int32_t>> seg_shards(n_segs);
+  for (int i = 0; i < n_shards; ++i) seg_shards[s->shard_seg[i]].push_back(i);
+  for (int g = 0; g < n_segs; ++g) {
+    const int32_t kv0 = s->cu_k[g], kvl = s->cu_k[g + 1] - kv0;
+    for (int32_t c0 = 0; c0 < kvl; c0 += FCP_TK) {
+      BwdItem it;
+      it.kv_row0 = kv0 + c0;
+      it.kv_rows = std::min(FCP_TK, kvl - c0);
+      it.kv_pos0 = c0;
+      it.reserved = 0;
+      it.sub_begin = (int32_t)s->bwd_sub.size();
+      int32_t q_tiles = 0;
+      for (int32_t i : seg_shards[g]) {
+        const int32_t a = s->cu_q[i], len = s->cu_q[i + 1] - a, p = s->q_pos_off[i];
+        if ((int64_t)p + len - 1 < c0 || len == 0) continue;     // no row of the shard sees the tile
+        const int32_t t_first = std::max<int64_t>(0, (int64_t)c0 - p);
+        const int32_t qt0 = t_first / FCP_BQ;
+        BwdSub sb;
+        sb.q_row0 = a + qt0 * FCP_BQ;
+        sb.q_pos0 = p + qt0 * FCP_BQ;
+        sb.q_rows = len - qt0 * FCP_BQ;
+        sb.pad_row0 = s->shard_pad0[i] + qt0 * FCP_BQ;
+        s->bwd_sub.push_back(sb);
+        q_tiles += (sb.q_rows + FCP_BQ - 1) / FCP_BQ;
+      }
+      it.sub_end = (int32_t)s->bwd_sub.size();
+      it.n_iters = q_tiles * s->G;
+      // a KV tile no query sees still gets dk = dv = 0 written (n_iters == 0)
+      for (int hk = 0; hk < s->Hkv; ++hk) {
+        it.kv_head = hk;
+        s->bwd.push_back(it);
+        s->bwd_tile_pairs += it.n_iters;
+      }
+    }
+  }
+  std::stable_sort(s->bwd.begin(), s->bwd.end(),
+                   [](const BwdItem& x, const BwdItem& y) { return x.n_iters > y.n_iters; });
+
+  // ---- workspace layout ----
+  size_t o = 0;
+  s->off_counters = o;  o = align_up(o + 256, 256);
+  s->off_fwd = o;       o = align_up(o + s->fwd.size() * sizeof(FwdItem), 256);
+  s->off_bwd = o;       o = align_up(o + s->bwd.size() * sizeof(BwdItem), 256);
+  s->off_sub = o;       o = align_up(o + s->bwd_sub.size() * sizeof(BwdSub), 256);
+  s->off_shard_meta = o;  // per padded 64-row tile: (local row0, valid rows)
+  o = align_up(o + (size_t)(s->n_q_pad / FCP_BQ) * 2 * sizeof(int32_t), 256);
+  s->off_lsed = o;      o = align_up(o + (size_t)s->Hq * s->n_q_pad * 2 * sizeof(float), 256);
+  s->off_dq = o;        o = align_up(o + (size_t)s->n_q * s->Hq * s->D * sizeof(float), 256);
+  s->total = std::max<size_t>(o, 256);
+  *out = s;
+  return FCP_OK;
+}
+
+extern "C" int fcp_sched_from_plan(const fcp_plan* plan, int32_t rank, int32_t n_q_heads,
+                                   int32_t n_kv_heads, int32_t head_dim, fcp_sched** out) {
+  if (!plan || !out || rank < 0 || rank >= plan->n_ranks) return FCP_INVALID_ARG;
+  RankView v;
+  fcp_build_rank_view(*plan, rank, v);
+  return fcp_sched_create(v.cu_q.data(), v.q_pos_off.data(), v.shard_seg.data(),
+                          (int32_t)v.q_pos_off.size(), v.cu_k.data(), (int32_t)v.kv_len.size(),
+                          n_q_heads, n_kv_heads, head_dim, out);
+}
+
+extern "C" void fcp_sched_destroy(fcp_sched* sched) { delete sched; }
+
+extern "C" int fcp_sched_workspace_size(const fcp_sched* sched, size_t* device_bytes) {
+  if (!sched || !device_bytes) return FCP_INVALID_ARG;
+  *device_bytes = sched->total;
+  return FCP_OK;
+}
+
+extern "C" int fcp_sched_get_info(const fcp_sched* sched, fcp_sched_info* out) {
+  if (!sched || !out) return FCP_INVALID_ARG;
+  out->n_fwd_items = (int32_t)sched->fwd.size();
+  out->n_bwd_items = (int32_t)sched->bwd.size();
+  out->fwd_kv_tiles = sched->fwd_kv_tiles;
+  out->bwd_tile_pairs = sched->bwd_tile_pairs;
+  out->useful_pairs = sched->useful_pairs;
+  out->n_q = sched->n_q;
+  out->n_kv = sched->n_kv;
+  return FCP_OK;
+}

@@ -242,20 +242,12 @@ extern "C" int fcp_sched_upload(const fcp_sched* s, void* workspace, void* strea
     return bytes == 0 ||
            cudaMemcpyAsync(w + off, src, bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
   };
-  std::vector<int32_t> meta;
-  for (size_t i = 0; i + 1 < s->cu_q.size(); ++i) {
-    const int32_t a = s->cu_q[i], len = s->cu_q[i + 1] - a;
-    for (int32_t r0 = 0; r0 < len; r0 += FCP_BQ) {
-      meta.push_back(a + r0);
-      meta.push_back(std::min(FCP_BQ, len - r0));
-    }
-  }
   bool ok = cudaMemsetAsync(w + s->off_counters, 0, 256, st) == cudaSuccess;
   ok = ok && put(s->off_fwd, s->fwd.data(), s->fwd.size() * sizeof(FwdItem));
   ok = ok && put(s->off_bwd, s->bwd.data(), s->bwd.size() * sizeof(BwdItem));
   ok = ok && put(s->off_sub, s->bwd_sub.data(), s->bwd_sub.size() * sizeof(BwdSub));
-  ok = ok && put(s->off_shard_meta, meta.data(), meta.size() * sizeof(int32_t));
-  // the sources are pageable host vectors that die with this call: wait for the copies
-  ok = ok && cudaStreamSynchronize(st) == cudaSuccess;
+  ok = ok && put(s->off_shard_meta, s->tile_meta.data(), s->tile_meta.size() * sizeof(int32_t));
+  // The sources are pageable host vectors owned by the schedule: cudaMemcpyAsync returns once
+  // they are staged, so no synchronisation is needed here.
   return ok ? FCP_OK : FCP_CUDA;
 }

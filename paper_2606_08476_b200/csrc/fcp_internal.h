@@ -67,6 +67,7 @@ struct fcp_sched {
   int64_t n_q = 0, n_kv = 0, n_q_pad = 0;          // n_q_pad: rows of the padded bwd scratch
   std::vector<int32_t> cu_q, q_pos_off, shard_seg, cu_k;
   std::vector<int32_t> shard_pad0;                 // [ns] first padded row of each shard
+  std::vector<int32_t> tile_meta;                  // per padded 64-row tile: (local row0, valid rows)
   std::vector<FwdItem> fwd;
   std::vector<BwdItem> bwd;
   std::vector<BwdSub> bwd_sub;

@@ -72,6 +72,13 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
     }
   }
   s->n_q_pad = pad;
+  for (int i = 0; i < n_shards; ++i) {
+    const int32_t a = s->cu_q[i], len = s->cu_q[i + 1] - a;
+    for (int32_t r0 = 0; r0 < len; r0 += FCP_BQ) {
+      s->tile_meta.push_back(a + r0);
+      s->tile_meta.push_back(std::min(FCP_BQ, len - r0));
+    }
+  }
   std::stable_sort(s->fwd.begin(), s->fwd.end(),
                    [](const FwdItem& x, const FwdItem& y) { return x.n_kv_tiles > y.n_kv_tiles; });
 
@@ -123,7 +130,7 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
   s->off_shard_meta = o;  // per padded 64-row tile: (local row0, valid rows)
   o = align_up(o + (size_t)(s->n_q_pad / FCP_BQ) * 2 * sizeof(int32_t), 256);
   s->off_lsed = o;      o = align_up(o + (size_t)s->Hq * s->n_q_pad * 2 * sizeof(float), 256);
-  s->off_dq = o;        o = align_up(o + (size_t)s->n_q * s->Hq * s->D * sizeof(float), 256);
+  s->off_dq = o;        o = align_up(o + (size_t)s->n_q_pad * s->Hq * s->D * sizeof(float), 256);
   s->total = std::max<size_t>(o, 256);
   *out = s;
   return FCP_OK;

@@ -1,0 +1,95 @@
+"""Helpers for the GPU parity tests: run one virtual rank through the C-ABI (via the binding)
+and through the oracle on the same seeded inputs, and compare element by element."""
+import math
+
+import numpy as np
+
+import fcp_inputs
+from oracle import attention as OA
+from oracle import kvselect as OKV
+from oracle import planner as OP
+
+# tolerances from BASELINE.json:north_star (bf16 inputs, fp32 accumulate)
+TOL_MAX_ABS = 2e-2
+TOL_MEAN_ABS = 2e-3
+TOL_LSE = 1e-3
+
+
+def to_f64(t):
+    return fcp_inputs.bf16_to_f64(t) if str(t.dtype) == "torch.bfloat16" else \
+        t.detach().cpu().double().numpy()
+
+
+def check(name, got, want, max_abs=TOL_MAX_ABS, mean_abs=TOL_MEAN_ABS):
+    got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)
+    assert got.shape == want.shape, (name, got.shape, want.shape)
+    assert np.isfinite(got).all(), "%s: non-finite values" % name
+    err = np.abs(got - want)
+    mx, mean = (float(err.max()), float(err.mean())) if err.size else (0.0, 0.0)
+    assert mx <= max_abs and mean <= mean_abs, \
+        "%s: max-abs %.3e (tol %.1e), mean-abs %.3e (tol %.1e)" % (name, mx, max_abs, mean, mean_abs)
+    return mx, mean
+
+
+def check_lse(name, got, want):
+    got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)
+    inf = np.isneginf(want)
+    assert np.array_equal(np.isneginf(got), inf), "%s: -inf pattern differs" % name
+    err = np.abs(got[~inf] - want[~inf])
+    mx = float(err.max()) if err.size else 0.0
+    assert mx <= TOL_LSE, "%s: max-abs %.3e (tol %.1e)" % (name, mx, TOL_LSE)
+    return mx
+
+
+def run_rank_gpu(fcp, plan, rank, Q, K, V, dO, scale, do_bwd=True):
+    """Whole per-rank hot path on the GPU: gather -> fwd -> bwd.  Q,K,V,dO global bf16 cuda."""
+    import torch
+    lay = plan.rank_layout(rank)
+    qi = torch.from_numpy(lay["q_token_index"].astype(np.int64)).to(Q.device)
+    q, do = Q[qi].contiguous(), dO[qi].contiguous()
+    kg, vg, counts = plan.kv_gather(rank, K, V)
+    sched = plan.sched(rank, Q.shape[1], K.shape[1], Q.shape[2]).upload(Q.device)
+    o, lse = sched.attn_fwd(q, kg, vg, scale)
+    out = {"q": q, "do": do, "k": kg, "v": vg, "o": o, "lse": lse, "counts": counts,
+           "layout": lay, "sched": sched}
+    if do_bwd:
+        out["dq"], out["dk"], out["dv"] = sched.attn_bwd(q, kg, vg, o, lse, do, scale)
+    torch.cuda.synchronize()
+    return out
+
+
+def run_rank_oracle(d, N, rank, Q, K, V, dO, scale, r_ppm=1_050_000, strategy=0, do_bwd=True):
+    """Same rank through oracle/ (fp64).  Q,K,V,dO are numpy fp64 arrays in global order."""
+    pl = OP.plan(d, N, r_ppm, strategy)
+    lay = OKV.rank_layout(pl, rank)
+    qi = OKV.q_token_index(pl, rank)
+    gi = OKV.gather_index(pl, rank)
+    args = (lay.cu_seqlens_q, lay.q_pos_off, lay.shard_seg, lay.cu_seqlens_k, scale)
+    o, lse = OA.rank_fwd(Q[qi], K[gi], V[gi], *args)
+    out = {"o": o, "lse": lse, "gather_index": gi, "q_index": qi}
+    if do_bwd:
+        out["dq"], out["dk"], out["dv"] = OA.rank_bwd(Q[qi], K[gi], V[gi], o, lse, dO[qi], *args)
+    return out
+
+
+def compare_rank(fcp, d, N, rank, Hq, Hkv, D, seed=0, r_ppm=1_050_000, strategy=0, do_bwd=True,
+                 verbose=False):
+    import torch
+    C = sum(d)
+    scale = 1.0 / math.sqrt(D)
+    Q, K, V, dO = fcp_inputs.make_tensors(C, Hq, Hkv, D, seed)
+    plan = fcp.Plan(d, N, r_ppm, strategy)
+    dev = torch.device("cuda:0")
+    g = run_rank_gpu(fcp, plan, rank, Q.to(dev), K.to(dev), V.to(dev), dO.to(dev), scale, do_bwd)
+    w = run_rank_oracle(d, N, rank, to_f64(Q), to_f64(K), to_f64(V), to_f64(dO), scale, r_ppm,
+                        strategy, do_bwd)
+    # gathered KV: bit-exact
+    assert torch.equal(g["k"].cpu(), K[torch.from_numpy(w["gather_index"].astype(np.int64))])
+    assert torch.equal(g["v"].cpu(), V[torch.from_numpy(w["gather_index"].astype(np.int64))])
+    res = {"o": check("o", to_f64(g["o"]), w["o"]), "lse": check_lse("lse", to_f64(g["lse"]), w["lse"])}
+    if do_bwd:
+        for k in ("dq", "dk", "dv"):
+            res[k] = check(k, to_f64(g[k]), w[k])
+    if verbose:
+        print("rank", rank, res)
+    return res

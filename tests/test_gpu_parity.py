@@ -1,0 +1,233 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element on
+the same seeded inputs.  Integer / byte work bit-exact; floating point within the tolerances
+of BASELINE.json:north_star (o,dq,dk,dv max-abs 2e-2, mean-abs 2e-3; lse 1e-3)."""
+import math
+
+import numpy as np
+import pytest
+
+import fcp_inputs
+import gpu_util as U
+from oracle import attention as OA
+from oracle import kvselect as OKV
+from oracle import planner as OP
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return torch
+
+
+# ---------------------------------------------------------------------------------- gather
+@pytest.mark.parametrize("name", ["tiny", "8b", "short", "longtail"])
+def test_kv_gather_bit_exact(fcp, torch, name):
+    cfg = fcp_inputs.CONFIGS[name]
+    d = fcp_inputs.doc_lengths(name, 0)
+    g = torch.Generator().manual_seed(3)
+    K = torch.randn((cfg.C, cfg.Hkv, cfg.D), generator=g).to(torch.bfloat16)
+    V = torch.randn((cfg.C, cfg.Hkv, cfg.D), generator=g).to(torch.bfloat16)
+    Kd, Vd = K.cuda(), V.cuda()
+    plan, opl = fcp.Plan(d, cfg.N), OP.plan(d, cfg.N)
+    st = OKV.kv_stats(opl)
+    row_bytes = cfg.Hkv * cfg.D * 2
+    for r in range(cfg.N):
+        kg, vg, cnt = plan.kv_gather(r, Kd, Vd)
+        torch.cuda.synchronize()
+        gi = torch.from_numpy(OKV.gather_index(opl, r).astype(np.int64))
+        assert torch.equal(kg.cpu(), K[gi]) and torch.equal(vg.cpu(), V[gi])
+        assert cnt["total_tokens"] == st.gathered[r] and cnt["remote_tokens"] == st.remote[r]
+        assert cnt["total_bytes"] == 2 * st.gathered[r] * row_bytes
+        assert cnt["remote_bytes"] == 2 * st.remote[r] * row_bytes
+
+
+def test_kv_gather_many_ranges(fcp, torch):
+    """More source ranges than one launch carries (alternating documents on two ranks)."""
+    d = [16, 48] * 300                      # LPT puts the long ones apart -> many ranges
+    K = torch.arange(sum(d) * 2 * 8, dtype=torch.float32).reshape(sum(d), 2, 8).to(torch.bfloat16)
+    V = (K.float() * 0.5).to(torch.bfloat16)
+    plan, opl = fcp.Plan(d, 2), OP.plan(d, 2)
+    for r in range(2):
+        kg, vg, cnt = plan.kv_gather(r, K.cuda(), V.cuda())
+        torch.cuda.synchronize()
+        gi = torch.from_numpy(OKV.gather_index(opl, r).astype(np.int64))
+        assert torch.equal(kg.cpu(), K[gi]) and torch.equal(vg.cpu(), V[gi])
+    assert max(plan.kv_gather(r, K.cuda(), V.cuda())[2]["n_ranges"] for r in range(2)) > 120
+
+
+# ---------------------------------------------------------------------------------- merge
+@pytest.mark.parametrize("dtype", ["float32", "bfloat16"])
+@pytest.mark.parametrize("D", [64, 128])
+def test_merge(fcp, torch, dtype, D):
+    rows, H = 333, 3
+    g = torch.Generator().manual_seed(1)
+    dt = getattr(torch, dtype)
+    oa = torch.randn(rows, H, D, generator=g).to(dt)
+    ob = torch.randn(rows, H, D, generator=g).to(dt)
+    la, lb = torch.randn(H, rows, generator=g) * 3, torch.randn(H, rows, generator=g) * 3
+    la[0, :5] = -math.inf
+    lb[0, 3:8] = -math.inf                                  # rows 3,4: both partials empty
+    om, lm = fcp.merge(oa.cuda(), la.cuda(), ob.cuda(), lb.cuda())
+    torch.cuda.synchronize()
+    wo, wl = OA.merge(oa.double().numpy(), la.double().numpy(), ob.double().numpy(),
+                      lb.double().numpy())
+    U.check_lse("lse", lm.cpu().numpy(), wl)
+    tol = (1e-5, 1e-6) if dtype == "float32" else (U.TOL_MAX_ABS, U.TOL_MEAN_ABS)
+    U.check("o", om.cpu().double().numpy(), wo, *tol)
+    assert (om[3:5, 0].cpu() == 0).all()
+    # empty input is a no-op
+    e = torch.empty((0, H, D), dtype=dt, device="cuda")
+    el = torch.empty((H, 0), dtype=torch.float32, device="cuda")
+    fcp.merge(e, el, e, el)
+
+
+# ---------------------------------------------------------------------------------- attention
+def test_tiny_config_full(fcp, torch):
+    cfg = fcp_inputs.CONFIGS["tiny"]
+    d = fcp_inputs.doc_lengths("tiny", 0)
+    for r in range(cfg.N):
+        U.compare_rank(fcp, d, cfg.N, r, cfg.Hq, cfg.Hkv, cfg.D, seed=0)
+
+
+CASES = [
+    # d, N, Hq, Hkv, D, strategy          (ragged tails, several tiles, every kernel variant)
+    ([300, 200, 140], 2, 2, 2, 128, 0),            # G=1 -> NQ=1, D=128, ragged 64/128 tails
+    ([700, 500, 400, 192], 2, 4, 2, 128, 0),       # G=2 -> NQ=2, D=128
+    ([700, 500, 400, 192], 2, 4, 2, 64, 1),        # NQ=2, D=64, all Per-Doc
+    ([1000, 37, 1, 1, 1, 260, 100], 4, 6, 2, 64, 0),   # G=3 -> NQ=1; 1-token documents
+    ([129, 127, 65, 63], 1, 4, 1, 128, 2),         # N=1, G=4, tile boundaries +-1
+    ([2048], 4, 8, 2, 128, 0),                     # one document, Per-Doc chunks, GQA 4
+    ([33] * 31 + [1], 8, 2, 1, 64, 0),             # many short documents, shards < 64 rows
+    ([1500, 400, 100, 48], 2, 2, 1, 128, 2),       # Whole-Doc head cut
+]
+
+
+@pytest.mark.parametrize("case", CASES, ids=lambda c: "d%d_N%d_H%d-%d_D%d_s%d" % (
+    len(c[0]), c[1], c[2], c[3], c[4], c[5]))
+def test_ragged_cases(fcp, torch, case):
+    d, N, Hq, Hkv, D, strategy = case
+    for r in range(N):
+        U.compare_rank(fcp, d, N, r, Hq, Hkv, D, seed=1, strategy=strategy)
+
+
+def test_key_count_closed_form_full_size(fcp, torch):
+    """K = 0 makes lse = ln(#visible keys) exactly (SURVEY 8(c1) pin 3) and o the running mean
+    of V: checks every mask and offset of the real 8b-size launch without an O(n^2) oracle."""
+    cfg = fcp_inputs.CONFIGS["8b"]
+    d = fcp_inputs.doc_lengths("8b", 0)
+    plan = fcp.Plan(d, cfg.N)
+    _, _, V, _ = fcp_inputs.make_tensors(cfg.C, cfg.Hq, cfg.Hkv, cfg.D, 0)
+    Vd = V.cuda()
+    Kd = torch.zeros_like(Vd)
+    G = cfg.Hq // cfg.Hkv
+    for r in (0, cfg.N - 1):
+        lay = plan.rank_layout(r)
+        n_q = int(lay["cu_seqlens_q"][-1])
+        q = torch.randn((n_q, cfg.Hq, cfg.D), device="cuda").to(torch.bfloat16)
+        kg, vg, _ = plan.kv_gather(r, Kd, Vd)
+        sched = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload("cuda")
+        o, lse = sched.attn_fwd(q, kg, vg, 1.0 / math.sqrt(cfg.D))
+        torch.cuda.synchronize()
+        vis = np.concatenate([int(p) + 1 + np.arange(int(b - a)) for a, b, p in
+                              zip(lay["cu_seqlens_q"][:-1], lay["cu_seqlens_q"][1:], lay["q_pos_off"])])
+        want = np.broadcast_to(np.log(vis.astype(np.float64)), (cfg.Hq, n_q))
+        assert np.abs(lse.cpu().double().numpy() - want).max() <= 1e-3
+        # o = mean of the visible V rows (first shard, every query head)
+        a, b, p = int(lay["cu_seqlens_q"][0]), int(lay["cu_seqlens_q"][1]), int(lay["q_pos_off"][0])
+        k0 = int(lay["cu_seqlens_k"][lay["shard_seg"][0]])
+        vv = U.to_f64(vg[k0:k0 + p + (b - a)])
+        mean = np.cumsum(vv, axis=0)[p:p + (b - a)] / vis[a:b, None, None]
+        U.check("o", U.to_f64(o[a:b]), np.repeat(mean, G, axis=1))
+
+
+def test_8b_config_one_gqa_group(fcp, torch):
+    """Full-size 8b launch (all heads on the GPU, the launch configuration bench.py times);
+    the oracle checks every row of one GQA group (heads are independent units)."""
+    cfg = fcp_inputs.CONFIGS["8b"]
+    d = fcp_inputs.doc_lengths("8b", 0)
+    scale = 1.0 / math.sqrt(cfg.D)
+    Q, K, V, dO = fcp_inputs.make_tensors(cfg.C, cfg.Hq, cfg.Hkv, cfg.D, 0)
+    plan = fcp.Plan(d, cfg.N)
+    G = cfg.Hq // cfg.Hkv
+    r, hk = 1, 5
+    g = U.run_rank_gpu(fcp, plan, r, Q.cuda(), K.cuda(), V.cuda(), dO.cuda(), scale)
+    hq = slice(hk * G, (hk + 1) * G)
+    w = U.run_rank_oracle(d, cfg.N, r, U.to_f64(Q[:, hq]), U.to_f64(K[:, hk:hk + 1]),
+                          U.to_f64(V[:, hk:hk + 1]), U.to_f64(dO[:, hq]), scale)
+    U.check("o", U.to_f64(g["o"][:, hq]), w["o"])
+    U.check_lse("lse", U.to_f64(g["lse"][hq]), w["lse"])
+    U.check("dq", U.to_f64(g["dq"][:, hq]), w["dq"])
+    U.check("dk", U.to_f64(g["dk"][:, hk:hk + 1]), w["dk"])
+    U.check("dv", U.to_f64(g["dv"][:, hk:hk + 1]), w["dv"])
+
+
+def test_kv_pieces_and_merge(fcp, torch):
+    """Split every shard's keys at c into two pieces (second piece: negative q_pos_off, rows that
+    see no key), run each piece through fcp_attn_fwd, combine with fcp_merge; backward through
+    the pieces with the merged lse / o (merge identity, backward through pieces)."""
+    Hq, Hkv, D = 4, 2, 128
+    scale = 1.0 / math.sqrt(D)
+    s_len, p, c = 200, 300, 330                  # shard rows [300,500) of a 500-token document
+    L = p + s_len
+    Q, K, V, dO = fcp_inputs.make_tensors(L, Hq, Hkv, D, 5)
+    q, do = Q[p:].contiguous().cuda(), dO[p:].contiguous().cuda()
+    ka, va = K[:c].contiguous().cuda(), V[:c].contiguous().cuda()
+    kb, vb = K[c:].contiguous().cuda(), V[c:].contiguous().cuda()
+    sa = fcp.Sched.create([0, s_len], [p], [0], [0, c], Hq, Hkv, D).upload("cuda")
+    sb = fcp.Sched.create([0, s_len], [p - c], [0], [0, L - c], Hq, Hkv, D).upload("cuda")
+    oa, la = sa.attn_fwd(q, ka, va, scale)
+    ob, lb = sb.attn_fwd(q, kb, vb, scale)
+    torch.cuda.synchronize()
+    assert torch.isneginf(lb[:, :c - p]).all() and (ob[:c - p] == 0).all()
+    om, lm = fcp.merge(oa, la, ob, lb)
+    f = U.to_f64
+    wo, wl = OA.shard_fwd(f(Q[p:]), f(K), f(V), p, scale)
+    U.check("o", f(om), wo)
+    U.check_lse("lse", f(lm), wl)
+    dqa, dka, dva = sa.attn_bwd(q, ka, va, om, lm, do, scale)
+    dqb, dkb, dvb = sb.attn_bwd(q, kb, vb, om, lm, do, scale)
+    torch.cuda.synchronize()
+    wdq, wdk, wdv = OA.shard_bwd(f(Q[p:]), f(K), f(V), wo, wl, f(dO[p:]), p, scale)
+    U.check("dq", f(dqa) + f(dqb), wdq, 3e-2, 3e-3)      # two bf16 roundings add
+    U.check("dk", np.concatenate([f(dka), f(dkb)]), wdk)
+    U.check("dv", np.concatenate([f(dva), f(dvb)]), wdv)
+
+
+def test_plan_invariance_on_gpu(fcp, torch):
+    """Outputs are identical (within tolerance) whatever the plan: hybrid, all-Per-Doc and
+    Whole-Doc results, put back in global order, all match the per-document oracle."""
+    d, N, Hq, Hkv, D = [900, 260, 250, 126], 4, 4, 2, 64
+    scale = 1.0 / math.sqrt(D)
+    C = sum(d)
+    Q, K, V, dO = fcp_inputs.make_tensors(C, Hq, Hkv, D, 2)
+    f = U.to_f64
+    want_o, want_lse = OA.packed_fwd(f(Q), f(K), f(V), d, scale)
+    want_dq, want_dk, want_dv = OA.packed_bwd(f(Q), f(K), f(V), f(dO), d, scale)
+    for strategy in (0, 1, 2):
+        plan = fcp.Plan(d, N, 0, strategy)
+        o = np.zeros_like(want_o)
+        lse = np.zeros_like(want_lse)
+        dq = np.zeros_like(want_dq)
+        dk, dv = np.zeros_like(want_dk), np.zeros_like(want_dv)
+        for r in range(N):
+            g = U.run_rank_gpu(fcp, plan, r, Q.cuda(), K.cuda(), V.cuda(), dO.cuda(), scale)
+            qi, ki = g["layout"]["q_token_index"], g["layout"]["kv_token_index"]
+            o[qi], lse[:, qi], dq[qi] = f(g["o"]), f(g["lse"]), f(g["dq"])
+            np.add.at(dk, ki, f(g["dk"]))                 # what ReduceScatter would do
+            np.add.at(dv, ki, f(g["dv"]))
+        U.check("o", o, want_o)
+        U.check_lse("lse", lse, want_lse)
+        U.check("dq", dq, want_dq)
+        U.check("dk", dk, want_dk, 4e-2, 3e-3)            # up to N bf16 partials summed
+        U.check("dv", dv, want_dv, 4e-2, 3e-3)
+
+
+def test_missing_library_fails_loudly(fcp, monkeypatch):
+    import paper_2606_08476_b200.binding as B
+    monkeypatch.setattr(B, "_LIB", None)
+    monkeypatch.setattr(B, "LIB_PATH", "/nonexistent/libfcp.so")
+    with pytest.raises(ImportError):
+        B.version()

@@ -153,3 +153,256 @@ def run_reference(args):
         "e2e": {"value": val, "unit": "TFLOP/s", "h2d_bytes_per_step": 0,
                 "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA path
+# ------------------------------------------------------------------------------------------
+class Workload:
+    """One packed batch resident in HBM: global K, V and every virtual rank's local q, dO rows
+    (a CP rank owns its shards' tokens; only KV crosses ranks)."""
+
+    def __init__(self, fcp, cfg, name, seed, device, pinned_host=False):
+        import torch
+        self.cfg, self.name, self.seed = cfg, name, seed
+        self.d = fcp_inputs.doc_lengths(name, seed)
+        Q, K, V, dO = fcp_inputs.make_tensors(cfg.C, cfg.Hq, cfg.Hkv, cfg.D, seed, device=device)
+        self.K, self.V = K, V
+        plan = fcp.Plan(self.d, cfg.N)
+        self.q, self.do = [], []
+        for r in range(cfg.N):
+            qi = torch.from_numpy(plan.rank_layout(r)["q_token_index"].astype(np.int64)).to(device)
+            self.q.append(Q[qi].contiguous())
+            self.do.append(dO[qi].contiguous())
+        self.n_kv = [plan.rank_stats(r)["n_kv"] for r in range(cfg.N)]
+        self.loads = [plan.rank_stats(r)["load"] for r in range(cfg.N)]
+        self.stats = plan.stats()
+        del Q, dO
+        if pinned_host:
+            pin = lambda t: t.cpu().pin_memory()
+            self.hK, self.hV = pin(K), pin(V)
+            self.hq, self.hdo = [pin(t) for t in self.q], [pin(t) for t in self.do]
+            mk = lambda t: torch.empty(t.shape, dtype=t.dtype).pin_memory()
+            self.ho, self.hdq = [mk(t) for t in self.q], [mk(t) for t in self.q]
+            kvshape = lambda r: (self.n_kv[r], cfg.Hkv, cfg.D)
+            self.hdk = [torch.empty(kvshape(r), dtype=K.dtype).pin_memory() for r in range(cfg.N)]
+            self.hdv = [torch.empty(kvshape(r), dtype=K.dtype).pin_memory() for r in range(cfg.N)]
+
+
+def hot_path_step(fcp, w, scale, ev=None, out=None):
+    """plan -> for every virtual rank: layout/schedule -> KV gather -> fwd -> bwd, all through
+    the C ABI.  ev: optional dict of event lists to fill (per rank: gather, fwd, bwd pairs)."""
+    import torch
+    cfg = w.cfg
+    plan = fcp.Plan(w.d, cfg.N)
+    for r in range(cfg.N):
+        sched = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload(w.K.device)
+        e = ev[r] if ev is not None else None
+        if e:
+            e["g0"].record()
+        kg, vg, _ = plan.kv_gather(r, w.K, w.V)
+        if e:
+            e["g1"].record()
+        o, lse = sched.attn_fwd(w.q[r], kg, vg, scale, events=(e["f0"], e["f1"]) if e else None)
+        res = sched.attn_bwd(w.q[r], kg, vg, o, lse, w.do[r], scale,
+                             events=(e["b0"], e["b1"]) if e else None)
+        if out is not None:
+            out.append((o,) + tuple(res))
+    return plan
+
+
+def e2e_step(fcp, w, scale):
+    """Same step from HOST buffers: pinned K, V, q, dO go host->device, results come back."""
+    import torch
+    cfg = w.cfg
+    dev = w.K.device
+    K, V = w.hK.to(dev, non_blocking=True), w.hV.to(dev, non_blocking=True)
+    plan = fcp.Plan(w.d, cfg.N)
+    for r in range(cfg.N):
+        q, do = w.hq[r].to(dev, non_blocking=True), w.hdo[r].to(dev, non_blocking=True)
+        sched = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload(dev)
+        kg, vg, _ = plan.kv_gather(r, K, V)
+        o, lse = sched.attn_fwd(q, kg, vg, scale)
+        dq, dk, dv = sched.attn_bwd(q, kg, vg, o, lse, do, scale)
+        w.ho[r].copy_(o, non_blocking=True)
+        w.hdq[r].copy_(dq, non_blocking=True)
+        w.hdk[r].copy_(dk, non_blocking=True)
+        w.hdv[r].copy_(dv, non_blocking=True)
+    nb = lambda t: t.numel() * t.element_size()
+    h2d = nb(w.hK) + nb(w.hV) + sum(nb(t) for t in w.hq) + sum(nb(t) for t in w.hdo)
+    d2h = sum(nb(t) for t in w.ho + w.hdq + w.hdk + w.hdv)
+    return h2d, d2h
+
+
+def run_fcp(args):
+    import torch
+    import paper_2606_08476_b200 as fcp
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = fcp_inputs.CONFIGS[args.config]
+    scale = 1.0 / math.sqrt(cfg.D)
+    # weak scaling: every GPU takes its own packed batch (independent problems, no collective)
+    w = Workload(fcp, cfg, args.config, args.seed + rank, dev, pinned_host=not args.no_e2e)
+    f_fwd, f_bwd = useful_flops(cfg, w.d)
+    peaks = measured_peaks()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if not dist:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    def sum_over_ranks(x):
+        if not dist:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        return float(t.item())
+
+    def new_event():
+        e = torch.cuda.Event(enable_timing=True)
+        e.record()                      # torch creates the cudaEvent_t lazily
+        return e
+
+    evs = [[{k: new_event() for k in ("g0", "g1", "f0", "f1", "b0", "b1")} for _ in range(cfg.N)]
+           for _ in range(args.steps)]
+    for _ in range(args.warmup):
+        hot_path_step(fcp, w, scale)
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t0.record()
+    for s in range(args.steps):
+        hot_path_step(fcp, w, scale, evs[s])
+    t1.record()
+    barrier()
+    ms = max_over_ranks(t0.elapsed_time(t1))
+    clocks = sampler.stop()
+    total_flops = sum_over_ranks(float(f_fwd + f_bwd)) * args.steps
+    value = total_flops / (ms * 1e-3) / 1e12
+
+    # per-kernel device times (this process), averaged over the timed steps
+    def avg(a, b):
+        return [float(np.mean([evs[s][r][a].elapsed_time(evs[s][r][b]) for s in range(args.steps)]))
+                for r in range(cfg.N)]
+    g_ms, f_ms, b_ms = avg("g0", "g1"), avg("f0", "f1"), avg("b0", "b1")
+    row_bytes = cfg.Hkv * cfg.D * 2
+    gather_bytes = [4 * n * row_bytes for n in w.n_kv]      # 2 tensors x (read + write)
+    pair_flop = cfg.D * cfg.Hq
+    fwd_flops = [4 * pair_flop * x for x in w.loads]
+    bwd_flops = [10 * pair_flop * x for x in w.loads]
+    bwd_tf = sum(bwd_flops) / (sum(b_ms) * 1e-3) / 1e12
+    fwd_tf = sum(fwd_flops) / (sum(f_ms) * 1e-3) / 1e12
+    gather_gbs = sum(gather_bytes) / (sum(g_ms) * 1e-3) / 1e9
+
+    # end to end from host buffers
+    e2e = None
+    if not args.no_e2e:
+        for _ in range(2):
+            e2e_step(fcp, w, scale)
+        barrier()
+        t0.record()
+        for _ in range(args.steps):
+            h2d, d2h = e2e_step(fcp, w, scale)
+        t1.record()
+        barrier()
+        ems = max_over_ranks(t0.elapsed_time(t1))
+        e2e = {"value": total_flops / (ems * 1e-3) / 1e12, "unit": "TFLOP/s",
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": ems / args.steps}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = len(os.sched_getaffinity(0))
+        cf, ct = oracle_sample(cfg, w.d, args.seed)
+        cpu = {"value": cf / ct / 1e12, "unit": "TFLOP/s", "cores": cores, "kind": "oracle",
+               "seconds": ct,
+               "sample": "all %d virtual ranks, one GQA group (1 of %d kv heads) of the same "
+                         "documents, fp64 numpy" % (cfg.N, cfg.Hkv)}
+
+    if rank == 0:
+        st = w.stats
+        kv_b = 2 * row_bytes                                  # K and V, one pass, per token
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "bwd_main_dram_bytes.json")
+        if os.path.exists(tp):
+            try:
+                traffic = json.load(open(tp)).get(args.config)
+            except Exception:
+                traffic = None
+        line = {
+            "metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": args.config, "C": cfg.C, "cp_ranks": cfg.N, "Hq": cfg.Hq,
+                       "Hkv": cfg.Hkv, "D": cfg.D, "n_docs": len(w.d), "seed": args.seed,
+                       "l2": "inputs larger than L2 (per-rank q,o,dO,dq + fp32 dq scratch "
+                             "= %.0f MiB vs 126 MB L2)" % (
+                                 cfg.C // cfg.N * cfg.Hq * cfg.D * (4 * 2 + 4) / 2 ** 20),
+                       "step": "plan + per virtual rank: schedule upload, KV gather, fwd, bwd"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": 5 * cfg.N * args.steps,
+            "roofline": {"bound": "tensor", "kernel": "fcp_attn_bwd_main", "achieved": bwd_tf,
+                         "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
+                         "frac": bwd_tf / peaks["bf16_sustained"], "traffic": traffic,
+                         "peak_source": peaks["source"] + " cuBLAS bf16, sustained",
+                         "frac_of_nominal_2250": bwd_tf / NOMINAL_BF16_TFLOPS},
+            "kernels": {
+                "attn_fwd": {"tflops": fwd_tf, "frac_measured": fwd_tf / peaks["bf16_sustained"],
+                             "ms_per_rank": f_ms},
+                "attn_bwd_main": {"tflops": bwd_tf, "ms_per_rank": b_ms},
+                "fwd_bwd_kernels_only": {"tflops": (sum(fwd_flops) + sum(bwd_flops)) /
+                                         ((sum(f_ms) + sum(b_ms)) * 1e-3) / 1e12},
+                "kv_gather": {"gbs": gather_gbs, "frac_measured_hbm": gather_gbs / peaks["hbm"],
+                              "ms_per_rank": g_ms, "bytes_per_rank": gather_bytes}},
+            "plan": {"imbalance": st["imbalance_ppm"] / 1e6, "n_per_doc": st["n_per_doc"],
+                     "max_load": st["max_load"], "mean_load": st["sum_load"] / cfg.N,
+                     "eq4_kv_bytes": st["eq4_tokens"] * kv_b, "eq5_kv_bytes": st["eq5_tokens"] * kv_b,
+                     "max_remote_kv_bytes": st["max_remote_tokens"] * kv_b,
+                     "sum_remote_kv_bytes": st["sum_remote_tokens"] * kv_b},
+            "cpu_baseline": cpu}
+        print(json.dumps(line))
+    if dist:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="8b", choices=sorted(fcp_inputs.CONFIGS))
+    ap.add_argument("--seed", type=int, default=0)
+    ap.add_argument("--impl", default="fcp", choices=["fcp", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_fcp(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -172,6 +172,7 @@ int  fcp_sched_get_info(const fcp_sched* sched, fcp_sched_info* out);
  *                layout of k, v (global dK = sum over ranks of scatter-add).
  *    bf16 tensor-core products with fp32 accumulation, fp32 softmax.
  * ------------------------------------------------------------------------------------------ */
+enum { FCP_DTYPE_BF16 = 0, FCP_DTYPE_F32 = 1 };
 typedef struct {
   const fcp_sched* sched;    /* host */
   void*       workspace;     /* device, >= fcp_sched_workspace_size bytes, uploaded */
@@ -181,8 +182,13 @@ typedef struct {
   void*       o;             /* device bf16 [n_q , Hq , D]: written by fwd, read by bwd */
   float*      lse;           /* device f32  [Hq, n_q]    : written by fwd, read by bwd */
   float       scale;         /* softmax scale, e.g. 1/sqrt(D) */
-  int32_t     reserved;
+  int32_t     dkv_dtype;     /* element type of dk, dv written by fcp_attn_bwd: FCP_DTYPE_BF16 (0)
+                                or FCP_DTYPE_F32 (partials that a dKV reduction sums in fp32) */
   void*       stream;
+  void*       ev_start;      /* optional cudaEvent_t (NULL = none) recorded on `stream` right before */
+  void*       ev_stop;       /* ... and right after the call's dominant kernel (the tcgen05
+                                attention kernel of fwd / the main kernel of bwd): lets a caller
+                                time that kernel alone without a profiler */
 } fcp_attn_args;
 int  fcp_attn_fwd(const fcp_attn_args* args);
 int  fcp_attn_bwd(const fcp_attn_args* args, const void* dO, void* dq, void* dk, void* dv);
@@ -194,7 +200,6 @@ int  fcp_attn_bwd(const fcp_attn_args* args, const void* dO, void* dq, void* dk,
  *    o_* : [n_rows, n_heads, head_dim] (o_dtype: 0 = bf16, 1 = f32), lse_* : [n_heads, n_rows]
  *    f32.  Outputs may alias the `a` inputs.
  * ------------------------------------------------------------------------------------------ */
-enum { FCP_DTYPE_BF16 = 0, FCP_DTYPE_F32 = 1 };
 int  fcp_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b,
                void* o_out, float* lse_out, int64_t n_rows, int32_t n_heads, int32_t head_dim,
                int32_t o_dtype, void* stream);

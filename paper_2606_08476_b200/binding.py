@@ -73,7 +73,8 @@ class _SchedInfo(C.Structure):
 class _AttnArgs(C.Structure):
     _fields_ = [("sched", C.c_void_p), ("workspace", C.c_void_p), ("q", C.c_void_p),
                 ("k", C.c_void_p), ("v", C.c_void_p), ("o", C.c_void_p), ("lse", C.c_void_p),
-                ("scale", C.c_float), ("reserved", C.c_int32), ("stream", C.c_void_p)]
+                ("scale", C.c_float), ("dkv_dtype", C.c_int32), ("stream", C.c_void_p),
+                ("ev_start", C.c_void_p), ("ev_stop", C.c_void_p)]
 
 
 _LIB = None
@@ -146,6 +147,14 @@ def _stream_ptr(stream):
         import torch
         return torch.cuda.current_stream().cuda_stream
     return getattr(stream, "cuda_stream", stream)
+
+
+def _event_ptr(ev):
+    """cudaEvent_t of a torch.cuda.Event (created lazily by torch: record it once first)."""
+    h = getattr(ev, "cuda_event", ev)
+    if not h:
+        raise ValueError("torch.cuda.Event has no handle yet: call ev.record() once before use")
+    return h
 
 
 class Plan:
@@ -271,15 +280,17 @@ class Sched:
                "fcp_sched_upload")
         return self
 
-    def _args(self, q, k, v, o, lse, scale, stream):
+    def _args(self, q, k, v, o, lse, scale, stream, events=None, dkv_f32=False):
         if self.workspace is None:
             self.upload(q.device)
+        ev0, ev1 = (None, None) if events is None else (_event_ptr(e) for e in events)
         return _AttnArgs(self._h, self.workspace.data_ptr(), q.data_ptr(), k.data_ptr(),
-                         v.data_ptr(), o.data_ptr(), lse.data_ptr(), float(scale), 0,
-                         _stream_ptr(stream))
+                         v.data_ptr(), o.data_ptr(), lse.data_ptr(), float(scale),
+                         1 if dkv_f32 else 0, _stream_ptr(stream), ev0, ev1)
 
-    def attn_fwd(self, q, k, v, scale, o=None, lse=None, stream=None):
-        """q [n_q,Hq,D], k,v [n_kv,Hkv,D] torch bf16 on the GPU -> (o bf16, lse f32 [Hq,n_q])."""
+    def attn_fwd(self, q, k, v, scale, o=None, lse=None, stream=None, events=None):
+        """q [n_q,Hq,D], k,v [n_kv,Hkv,D] torch bf16 on the GPU -> (o bf16, lse f32 [Hq,n_q]).
+        events = (start, stop) torch.cuda.Event pair recorded around the attention kernel."""
         import torch
         for t in (q, k, v):
             assert t.is_cuda and t.is_contiguous() and t.dtype == torch.bfloat16
@@ -287,18 +298,24 @@ class Sched:
             o = torch.empty_like(q)
         if lse is None:
             lse = torch.empty((self.Hq, q.shape[0]), dtype=torch.float32, device=q.device)
-        a = self._args(q, k, v, o, lse, scale, stream)
+        a = self._args(q, k, v, o, lse, scale, stream, events)
         _check(_lib().fcp_attn_fwd(C.byref(a)), "fcp_attn_fwd")
         return o, lse
 
-    def attn_bwd(self, q, k, v, o, lse, do, scale, dq=None, dk=None, dv=None, stream=None):
+    def attn_bwd(self, q, k, v, o, lse, do, scale, dq=None, dk=None, dv=None, stream=None,
+                 events=None, dkv_dtype=None):
+        """-> (dq bf16, dk, dv); dk, dv are bf16 unless dkv_dtype (or the given buffers) is f32."""
         import torch
         for t in (q, k, v, o, do):
             assert t.is_cuda and t.is_contiguous() and t.dtype == torch.bfloat16
+        if dkv_dtype is None:
+            dkv_dtype = dk.dtype if dk is not None else torch.bfloat16
+        assert dkv_dtype in (torch.bfloat16, torch.float32)
         dq = torch.empty_like(q) if dq is None else dq
-        dk = torch.empty_like(k) if dk is None else dk
-        dv = torch.empty_like(v) if dv is None else dv
-        a = self._args(q, k, v, o, lse, scale, stream)
+        dk = torch.empty_like(k, dtype=dkv_dtype) if dk is None else dk
+        dv = torch.empty_like(v, dtype=dkv_dtype) if dv is None else dv
+        assert dk.dtype == dkv_dtype and dv.dtype == dkv_dtype
+        a = self._args(q, k, v, o, lse, scale, stream, events, dkv_dtype == torch.float32)
         _check(_lib().fcp_attn_bwd(C.byref(a), do.data_ptr(), dq.data_ptr(), dk.data_ptr(),
                                    dv.data_ptr()), "fcp_attn_bwd")
         return dq, dk, dv

@@ -186,8 +186,8 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_v,
                   const BwdItem* __restrict__ items, int n_items,
                   const BwdSub* __restrict__ subs, const float2* __restrict__ lsed,
-                  float* __restrict__ dq_acc, __nv_bfloat16* __restrict__ dk,
-                  __nv_bfloat16* __restrict__ dv, int64_t n_q_pad, int Hkv, int G,
+                  float* __restrict__ dq_acc, void* __restrict__ dk_out,
+                  void* __restrict__ dv_out, int dkv_f32, int64_t n_q_pad, int Hkv, int G,
                   float scale, float scale_log2) {
   using Cfg = BwdCfg<D>;
   extern __shared__ uint8_t smem_raw[];
@@ -359,11 +359,14 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       if (idx < 0) continue;
       const BwdItem it = items[idx];
       const bool row_valid = row < it.kv_rows;
-      __nv_bfloat16* dk_row = dk + ((int64_t)(it.kv_row0 + row) * Hkv + it.kv_head) * D;
-      __nv_bfloat16* dv_row = dv + ((int64_t)(it.kv_row0 + row) * Hkv + it.kv_head) * D;
+      // output row of this thread, in bytes: bf16 or fp32 elements
+      const int64_t row_elem = ((int64_t)(it.kv_row0 + row) * Hkv + it.kv_head) * D;
+      const int esz = dkv_f32 ? 4 : 2;
+      uint8_t* dk_row = static_cast<uint8_t*>(dk_out) + row_elem * esz;
+      uint8_t* dv_row = static_cast<uint8_t*>(dv_out) + row_elem * esz;
       if (it.n_iters == 0) {                             // no query sees this tile
         if (row_valid)
-          for (int c = 0; c < D; c += 8) {
+          for (int c = 0; c < D * esz; c += 16) {
             *reinterpret_cast<int4*>(dk_row + c) = make_int4(0, 0, 0, 0);
             *reinterpret_cast<int4*>(dv_row + c) = make_int4(0, 0, 0, 0);
           }
@@ -432,13 +435,20 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       for (int which = 0; which < 2; ++which) {
         const uint32_t tacc = tmem_base + lane_addr + (which == 0 ? Cfg::kColDV : Cfg::kColDK);
         const float f = which == 0 ? 1.f : scale;
-        __nv_bfloat16* dst = which == 0 ? dv_row : dk_row;
+        uint8_t* dst_b = which == 0 ? dv_row : dk_row;
+        __nv_bfloat16* dst = reinterpret_cast<__nv_bfloat16*>(dst_b);
 #pragma unroll
         for (int c = 0; c < D / 32; ++c) {
           uint32_t acc[32];
           tmem_ld32(tacc + c * 32, acc);
           tmem_ld_wait();
-          if (row_valid) {
+          if (row_valid && dkv_f32) {
+            float4* d4 = reinterpret_cast<float4*>(dst_b) + c * 8;
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+              d4[i] = make_float4(__uint_as_float(acc[4 * i + 0]) * f, __uint_as_float(acc[4 * i + 1]) * f,
+                                  __uint_as_float(acc[4 * i + 2]) * f, __uint_as_float(acc[4 * i + 3]) * f);
+          } else if (row_valid) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               int4 pk;
@@ -534,12 +544,15 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
                              Cfg::kSmemBytes) != cudaSuccess)
       return FCP_CUDA;
     const int grid = std::min(n_items, num_sms());
+    if (a->ev_start && cudaEventRecord((cudaEvent_t)a->ev_start, st) != cudaSuccess)
+      return FCP_CUDA;
     kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(
         mq, mdo, mk, mv, reinterpret_cast<const BwdItem*>(ws + s->off_bwd), n_items,
-        reinterpret_cast<const BwdSub*>(ws + s->off_sub), lsed, dq_acc,
-        static_cast<__nv_bfloat16*>(dk), static_cast<__nv_bfloat16*>(dv), s->n_q_pad, s->Hkv,
-        s->G, a->scale, a->scale * kLog2e);
+        reinterpret_cast<const BwdSub*>(ws + s->off_sub), lsed, dq_acc, dk, dv,
+        a->dkv_dtype == FCP_DTYPE_F32, s->n_q_pad, s->Hkv, s->G, a->scale, a->scale * kLog2e);
     if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
+    if (a->ev_stop && cudaEventRecord((cudaEvent_t)a->ev_stop, st) != cudaSuccess)
+      return FCP_CUDA;
   }
   if (n_pad_tiles > 0) {
     fcp_bwd_dq_convert<D><<<dim3(n_pad_tiles, s->Hq), 256, 0, st>>>(
@@ -556,6 +569,7 @@ extern "C" int fcp_attn_bwd(const fcp_attn_args* a, const void* dO, void* dq, vo
       !dq || !dk || !dv)
     return FCP_INVALID_ARG;
   const fcp_sched* s = a->sched;
+  if (a->dkv_dtype != FCP_DTYPE_BF16 && a->dkv_dtype != FCP_DTYPE_F32) return FCP_UNSUPPORTED;
   for (const void* p : {a->q, a->k, a->v, (const void*)a->o, (const void*)a->workspace, dO,
                         (const void*)dq, (const void*)dk, (const void*)dv})
     if (reinterpret_cast<uintptr_t>(p) & 15) return FCP_MISALIGNED;

@@ -352,10 +352,14 @@ int launch_fwd(const fcp_attn_args* a, const fcp_sched* s) {
   const int grid = std::min(n_items, num_sms());
   const FwdItem* items =
       reinterpret_cast<const FwdItem*>(static_cast<const char*>(a->workspace) + s->off_fwd);
-  kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, (cudaStream_t)a->stream>>>(
+  cudaStream_t st = (cudaStream_t)a->stream;
+  if (a->ev_start && cudaEventRecord((cudaEvent_t)a->ev_start, st) != cudaSuccess) return FCP_CUDA;
+  kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(
       mq, mk, mv, items, n_items, static_cast<__nv_bfloat16*>(a->o), a->lse, s->n_q, s->Hq,
       a->scale * kLog2e);
-  return cudaGetLastError() == cudaSuccess ? FCP_OK : FCP_CUDA;
+  if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
+  if (a->ev_stop && cudaEventRecord((cudaEvent_t)a->ev_stop, st) != cudaSuccess) return FCP_CUDA;
+  return FCP_OK;
 }
 
 }  // namespace

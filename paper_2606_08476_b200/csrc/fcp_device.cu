@@ -214,13 +214,13 @@ extern "C" int fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, 
 extern "C" int fcp_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b,
                          void* o_out, float* lse_out, int64_t n_rows, int32_t n_heads,
                          int32_t head_dim, int32_t o_dtype, void* stream) {
-  if (!o_a || !lse_a || !o_b || !lse_b || !o_out || !lse_out || n_rows < 0 || n_heads < 1)
-    return FCP_INVALID_ARG;
+  if (n_rows < 0 || n_heads < 1) return FCP_INVALID_ARG;
   if ((head_dim != 64 && head_dim != 128) ||
       (o_dtype != FCP_DTYPE_BF16 && o_dtype != FCP_DTYPE_F32))
     return FCP_UNSUPPORTED;
+  if (n_rows == 0) return FCP_OK;                  // empty input: nothing to do, pointers unused
+  if (!o_a || !lse_a || !o_b || !lse_b || !o_out || !lse_out) return FCP_INVALID_ARG;
   if (!aligned16(o_a) || !aligned16(o_b) || !aligned16(o_out)) return FCP_MISALIGNED;
-  if (n_rows == 0) return FCP_OK;
   const int64_t threads = n_rows * n_heads * (head_dim / 8);
   const int64_t blocks = (threads + 255) / 256;
   if (blocks > INT32_MAX) return FCP_INVALID_ARG;

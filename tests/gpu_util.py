@@ -20,14 +20,29 @@ def to_f64(t):
         t.detach().cpu().double().numpy()
 
 
-def check(name, got, want, max_abs=TOL_MAX_ABS, mean_abs=TOL_MEAN_ABS):
+def bf16_half_ulp(x):
+    """Largest error of rounding x to bf16 (8 significant bits): 2^(floor(log2|x|) - 8)."""
+    ax = np.abs(np.asarray(x, dtype=np.float64))
+    e = np.floor(np.log2(np.maximum(ax, 2.0 ** -126)))
+    return np.where(ax > 0, 2.0 ** (e - 8), 0.0)
+
+
+def check(name, got, want, max_abs=TOL_MAX_ABS, mean_abs=TOL_MEAN_ABS, bf16_sum=False):
+    """north_star tolerances.  bf16_sum=True is for dk/dv written as bf16: they are sums over
+    many queries and G heads whose magnitude exceeds 8, where rounding the exact value to bf16
+    alone costs up to 2^-5 = 3.1e-2 > 2e-2; the per-element bound is then max_abs + the bf16
+    half-ulp of the expected value.  The fp32-output mode of the same
+    kernel is held to the plain max_abs."""
     got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)
     assert got.shape == want.shape, (name, got.shape, want.shape)
     assert np.isfinite(got).all(), "%s: non-finite values" % name
     err = np.abs(got - want)
     mx, mean = (float(err.max()), float(err.mean())) if err.size else (0.0, 0.0)
-    assert mx <= max_abs and mean <= mean_abs, \
-        "%s: max-abs %.3e (tol %.1e), mean-abs %.3e (tol %.1e)" % (name, mx, max_abs, mean, mean_abs)
+    bound = max_abs + (bf16_half_ulp(want) if bf16_sum else 0.0)
+    worst = float((err - bound).max()) if err.size else -1.0
+    assert worst <= 0 and mean <= mean_abs, \
+        "%s: max-abs %.3e (tol %.1e%s), mean-abs %.3e (tol %.1e)" % (
+            name, mx, max_abs, " + bf16 half-ulp" if bf16_sum else "", mean, mean_abs)
     return mx, mean
 
 
@@ -41,7 +56,7 @@ def check_lse(name, got, want):
     return mx
 
 
-def run_rank_gpu(fcp, plan, rank, Q, K, V, dO, scale, do_bwd=True):
+def run_rank_gpu(fcp, plan, rank, Q, K, V, dO, scale, do_bwd=True, dkv_f32=False):
     """Whole per-rank hot path on the GPU: gather -> fwd -> bwd.  Q,K,V,dO global bf16 cuda."""
     import torch
     lay = plan.rank_layout(rank)
@@ -53,7 +68,8 @@ def run_rank_gpu(fcp, plan, rank, Q, K, V, dO, scale, do_bwd=True):
     out = {"q": q, "do": do, "k": kg, "v": vg, "o": o, "lse": lse, "counts": counts,
            "layout": lay, "sched": sched}
     if do_bwd:
-        out["dq"], out["dk"], out["dv"] = sched.attn_bwd(q, kg, vg, o, lse, do, scale)
+        out["dq"], out["dk"], out["dv"] = sched.attn_bwd(
+            q, kg, vg, o, lse, do, scale, dkv_dtype=torch.float32 if dkv_f32 else torch.bfloat16)
     torch.cuda.synchronize()
     return out
 
@@ -73,14 +89,15 @@ def run_rank_oracle(d, N, rank, Q, K, V, dO, scale, r_ppm=1_050_000, strategy=0,
 
 
 def compare_rank(fcp, d, N, rank, Hq, Hkv, D, seed=0, r_ppm=1_050_000, strategy=0, do_bwd=True,
-                 verbose=False):
+                 verbose=False, dkv_f32=False):
     import torch
     C = sum(d)
     scale = 1.0 / math.sqrt(D)
     Q, K, V, dO = fcp_inputs.make_tensors(C, Hq, Hkv, D, seed)
     plan = fcp.Plan(d, N, r_ppm, strategy)
     dev = torch.device("cuda:0")
-    g = run_rank_gpu(fcp, plan, rank, Q.to(dev), K.to(dev), V.to(dev), dO.to(dev), scale, do_bwd)
+    g = run_rank_gpu(fcp, plan, rank, Q.to(dev), K.to(dev), V.to(dev), dO.to(dev), scale, do_bwd,
+                     dkv_f32)
     w = run_rank_oracle(d, N, rank, to_f64(Q), to_f64(K), to_f64(V), to_f64(dO), scale, r_ppm,
                         strategy, do_bwd)
     # gathered KV: bit-exact
@@ -88,8 +105,9 @@ def compare_rank(fcp, d, N, rank, Hq, Hkv, D, seed=0, r_ppm=1_050_000, strategy=
     assert torch.equal(g["v"].cpu(), V[torch.from_numpy(w["gather_index"].astype(np.int64))])
     res = {"o": check("o", to_f64(g["o"]), w["o"]), "lse": check_lse("lse", to_f64(g["lse"]), w["lse"])}
     if do_bwd:
-        for k in ("dq", "dk", "dv"):
-            res[k] = check(k, to_f64(g[k]), w[k])
+        res["dq"] = check("dq", to_f64(g["dq"]), w["dq"])
+        for k in ("dk", "dv"):
+            res[k] = check(k, to_f64(g[k]), w[k], bf16_sum=not dkv_f32)
     if verbose:
         print("rank", rank, res)
     return res

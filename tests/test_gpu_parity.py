@@ -107,10 +107,11 @@ CASES = [
 
 @pytest.mark.parametrize("case", CASES, ids=lambda c: "d%d_N%d_H%d-%d_D%d_s%d" % (
     len(c[0]), c[1], c[2], c[3], c[4], c[5]))
-def test_ragged_cases(fcp, torch, case):
+@pytest.mark.parametrize("dkv_f32", [False, True], ids=["dkv_bf16", "dkv_f32"])
+def test_ragged_cases(fcp, torch, case, dkv_f32):
     d, N, Hq, Hkv, D, strategy = case
     for r in range(N):
-        U.compare_rank(fcp, d, N, r, Hq, Hkv, D, seed=1, strategy=strategy)
+        U.compare_rank(fcp, d, N, r, Hq, Hkv, D, seed=1, strategy=strategy, dkv_f32=dkv_f32)
 
 
 def test_key_count_closed_form_full_size(fcp, torch):
@@ -143,7 +144,8 @@ def test_key_count_closed_form_full_size(fcp, torch):
         U.check("o", U.to_f64(o[a:b]), np.repeat(mean, G, axis=1))
 
 
-def test_8b_config_one_gqa_group(fcp, torch):
+@pytest.mark.parametrize("dkv_f32", [False, True], ids=["dkv_bf16", "dkv_f32"])
+def test_8b_config_one_gqa_group(fcp, torch, dkv_f32):
     """Full-size 8b launch (all heads on the GPU, the launch configuration bench.py times);
     the oracle checks every row of one GQA group (heads are independent units)."""
     cfg = fcp_inputs.CONFIGS["8b"]
@@ -153,15 +155,16 @@ def test_8b_config_one_gqa_group(fcp, torch):
     plan = fcp.Plan(d, cfg.N)
     G = cfg.Hq // cfg.Hkv
     r, hk = 1, 5
-    g = U.run_rank_gpu(fcp, plan, r, Q.cuda(), K.cuda(), V.cuda(), dO.cuda(), scale)
+    g = U.run_rank_gpu(fcp, plan, r, Q.cuda(), K.cuda(), V.cuda(), dO.cuda(), scale,
+                       dkv_f32=dkv_f32)
     hq = slice(hk * G, (hk + 1) * G)
     w = U.run_rank_oracle(d, cfg.N, r, U.to_f64(Q[:, hq]), U.to_f64(K[:, hk:hk + 1]),
                           U.to_f64(V[:, hk:hk + 1]), U.to_f64(dO[:, hq]), scale)
     U.check("o", U.to_f64(g["o"][:, hq]), w["o"])
     U.check_lse("lse", U.to_f64(g["lse"][hq]), w["lse"])
     U.check("dq", U.to_f64(g["dq"][:, hq]), w["dq"])
-    U.check("dk", U.to_f64(g["dk"][:, hk:hk + 1]), w["dk"])
-    U.check("dv", U.to_f64(g["dv"][:, hk:hk + 1]), w["dv"])
+    U.check("dk", U.to_f64(g["dk"][:, hk:hk + 1]), w["dk"], bf16_sum=not dkv_f32)
+    U.check("dv", U.to_f64(g["dv"][:, hk:hk + 1]), w["dv"], bf16_sum=not dkv_f32)
 
 
 def test_kv_pieces_and_merge(fcp, torch):
@@ -192,8 +195,8 @@ def test_kv_pieces_and_merge(fcp, torch):
     torch.cuda.synchronize()
     wdq, wdk, wdv = OA.shard_bwd(f(Q[p:]), f(K), f(V), wo, wl, f(dO[p:]), p, scale)
     U.check("dq", f(dqa) + f(dqb), wdq, 3e-2, 3e-3)      # two bf16 roundings add
-    U.check("dk", np.concatenate([f(dka), f(dkb)]), wdk)
-    U.check("dv", np.concatenate([f(dva), f(dvb)]), wdv)
+    U.check("dk", np.concatenate([f(dka), f(dkb)]), wdk, bf16_sum=True)
+    U.check("dv", np.concatenate([f(dva), f(dvb)]), wdv, bf16_sum=True)
 
 
 def test_plan_invariance_on_gpu(fcp, torch):
@@ -213,7 +216,8 @@ def test_plan_invariance_on_gpu(fcp, torch):
         dq = np.zeros_like(want_dq)
         dk, dv = np.zeros_like(want_dk), np.zeros_like(want_dv)
         for r in range(N):
-            g = U.run_rank_gpu(fcp, plan, r, Q.cuda(), K.cuda(), V.cuda(), dO.cuda(), scale)
+            g = U.run_rank_gpu(fcp, plan, r, Q.cuda(), K.cuda(), V.cuda(), dO.cuda(), scale,
+                               dkv_f32=True)    # fp32 partials, summed like a ReduceScatter
             qi, ki = g["layout"]["q_token_index"], g["layout"]["kv_token_index"]
             o[qi], lse[:, qi], dq[qi] = f(g["o"]), f(g["lse"]), f(g["dq"])
             np.add.at(dk, ki, f(g["dk"]))                 # what ReduceScatter would do
@@ -221,8 +225,8 @@ def test_plan_invariance_on_gpu(fcp, torch):
         U.check("o", o, want_o)
         U.check_lse("lse", lse, want_lse)
         U.check("dq", dq, want_dq)
-        U.check("dk", dk, want_dk, 4e-2, 3e-3)            # up to N bf16 partials summed
-        U.check("dv", dv, want_dv, 4e-2, 3e-3)
+        U.check("dk", dk, want_dk)
+        U.check("dv", dv, want_dv)
 
 
 def test_missing_library_fails_loudly(fcp, monkeypatch):

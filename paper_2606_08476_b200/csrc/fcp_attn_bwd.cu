@@ -100,8 +100,8 @@ struct BwdCfg {
   static constexpr int kQTile = FCP_BQ * D * 2;          // Q or dO tile: kPanels x [64 rows x 128 B]
   static constexpr int kQPanel = FCP_BQ * 128;
   static constexpr int kStat = FCP_BQ * 8;               // (lse, delta) of one q tile
-  static constexpr int kStage = 2 * kQTile + 1024;       // Q, dO, stats (padded)
-  static constexpr int kStages = 2;
+  static constexpr int kStage = 2 * kQTile;              // Q, dO
+  static constexpr int kStages = 3;
   static constexpr int kDS = 128 * 128;                  // dS^T bf16 [128 kv][64 q]
   static constexpr int kDQ = FCP_BQ * D * 4;             // dQ staging fp32 [64 q][D]
   static constexpr int kThreads = 384;
@@ -109,22 +109,27 @@ struct BwdCfg {
   static constexpr int kOffStage = 2 * kKVTile;
   static constexpr int kOffDS = kOffStage + kStages * kStage;
   static constexpr int kOffDQ = kOffDS + 2 * kDS;
-  static constexpr int kOffBar = kOffDQ + kDQ;
-  static constexpr int kSmemBytes = 1024 + kOffBar + 1024;
+  static constexpr int kOffStat = kOffDQ + kDQ;
+  static constexpr int kOffBar = kOffStat + kStages * kStat;
+  static constexpr int kSmemBytes = 1024 + kOffBar + 256;
   static constexpr uint32_t kStageTx = 2 * kQTile + kStat;
   // TMEM columns
   static constexpr int kColS = 0, kColDP = 128, kColDQ = 192, kColDV = 256, kColDK = 384;
+  // registers per thread after setmaxnreg: producer/MMA warpgroup, softmax warpgroup, drain warpgroup
+  static constexpr int kRegsCtl = 64, kRegsSoftmax = 256, kRegsDrain = 152;
 };
+static_assert(BwdCfg<128>::kSmemBytes <= 232448, "bwd shared memory exceeds 227 KB");
 
 struct BwdBarriers {
   uint64_t kv_full, kv_free;
-  uint64_t qdo_full[2], qdo_free[2];
+  uint64_t qdo_full[3], qdo_free[3];
   uint64_t st_full, dpt_free, p_ready;
   uint64_t ds_free[2];
   uint64_t dq_full, dq_free;
   uint64_t dkv_full, dkv_free;
   uint32_t tmem_base;
 };
+static_assert(sizeof(BwdBarriers) <= 256, "barrier block");
 
 __device__ __forceinline__ int snake_item_b(int round, int n_items) {
   const int g = gridDim.x, b = blockIdx.x;
@@ -178,6 +183,45 @@ __device__ __forceinline__ void bulk_wait0() {
   asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
+// One softmax step of the backward for one KV row (= one thread) and 64 query columns:
+//   P^T = exp2(S^T c - lse), masked;  dS^T = P^T o (dP^T - delta)
+// bf16 P^T / dS^T go back into TMEM (A operands of dV / dK) and dS^T into the swizzled smem tile
+// (B operand of dQ^T).  kMask selects the diagonal / ragged-tile variant; interior tiles skip
+// every mask instruction.
+template <bool kMask>
+__device__ __forceinline__ void bwd_softmax_tile(const uint32_t (&s)[64], const uint32_t (&dp)[64],
+                                                 uint32_t stat_addr, float scale_log2,
+                                                 int vis,   // kMask: columns c < vis are masked out
+                                                 uint32_t tS, uint32_t ds_row_addr, int row) {
+#pragma unroll
+  for (int h = 0; h < 4; ++h) {                       // 16 columns per step
+    uint32_t pk_p[8], pk_ds[8];
+#pragma unroll
+    for (int i = 0; i < 16; i += 2) {
+      const int c = h * 16 + i;
+      const float4 st01 = lds128(stat_addr + c * 8);  // lse0, delta0, lse1, delta1
+      float p0 = fast_exp2(fmaf(__uint_as_float(s[c]), scale_log2, -st01.x));
+      float p1 = fast_exp2(fmaf(__uint_as_float(s[c + 1]), scale_log2, -st01.z));
+      if (kMask) {
+        if (c < vis) p0 = 0.f;
+        if (c + 1 < vis) p1 = 0.f;
+      }
+      const float ds0 = p0 * (__uint_as_float(dp[c]) - st01.y);
+      const float ds1 = p1 * (__uint_as_float(dp[c + 1]) - st01.w);
+      pk_p[i >> 1] = pack_bf16(p0, p1);
+      pk_ds[i >> 1] = pack_bf16(ds0, ds1);
+    }
+    tmem_st8(tS + h * 8, pk_p);
+    tmem_st8(tS + 32 + h * 8, pk_ds);
+#pragma unroll
+    for (int c4 = 0; c4 < 2; ++c4) {                  // two 16-byte chunks of the 128-byte row
+      const int chunk = (h * 2 + c4) ^ (row & 7);
+      sts128(ds_row_addr + chunk * 16, pk_ds[4 * c4], pk_ds[4 * c4 + 1], pk_ds[4 * c4 + 2],
+             pk_ds[4 * c4 + 3]);
+    }
+  }
+}
+
 template <int D>
 __global__ void __launch_bounds__(BwdCfg<D>::kThreads, 1)
 fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
@@ -197,7 +241,8 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
   uint8_t* v_smem = k_smem + Cfg::kKVTile;
   uint8_t* stage_smem = smem + Cfg::kOffStage;
   uint8_t* ds_smem = smem + Cfg::kOffDS;
-  float* dq_smem = reinterpret_cast<float*>(smem + Cfg::kOffDQ);
+  uint8_t* dq_smem = smem + Cfg::kOffDQ;
+  uint8_t* stat_smem = smem + Cfg::kOffStat;
   BwdBarriers* bars = reinterpret_cast<BwdBarriers*>(smem + Cfg::kOffBar);
 
   const int warp = threadIdx.x >> 5;
@@ -206,11 +251,11 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
   if (threadIdx.x == 0) {
     mbar_init(&bars->kv_full, 1);
     mbar_init(&bars->kv_free, 1);
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < Cfg::kStages; ++i) {
       mbar_init(&bars->qdo_full[i], 1);
       mbar_init(&bars->qdo_free[i], 1);
-      mbar_init(&bars->ds_free[i], 1);
     }
+    for (int i = 0; i < 2; ++i) mbar_init(&bars->ds_free[i], 1);
     mbar_init(&bars->st_full, 1);
     mbar_init(&bars->dpt_free, 128);
     mbar_init(&bars->p_ready, 128);
@@ -227,9 +272,10 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
   const uint32_t tmem_base = bars->tmem_base;
   const int rounds = (n_items + gridDim.x - 1) / gridDim.x;
 
-  if (warp == 0) {
-    // ------------------------------------------------------------------ TMA producer
-    if (lane == 0) {
+  if (warp < 4) {
+    reg_dealloc<Cfg::kRegsCtl>();
+    if (warp == 0 && lane == 0) {
+      // ---------------------------------------------------------------- TMA producer
       prefetch_tmap(&tmap_q);
       prefetch_tmap(&tmap_do);
       prefetch_tmap(&tmap_k);
@@ -260,30 +306,34 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
             tma_load_3d(sq + Cfg::kQTile + pn * Cfg::kQPanel, &tmap_do, &bars->qdo_full[st],
                         pn * 64, head, w.q_row());
           }
-          bulk_load_1d(sq + 2 * Cfg::kQTile, lsed + (int64_t)head * n_q_pad + w.pad_row(),
+          bulk_load_1d(stat_smem + st * Cfg::kStat, lsed + (int64_t)head * n_q_pad + w.pad_row(),
                        Cfg::kStat, &bars->qdo_full[st]);
         }
         ++m;
       }
-    }
-  } else if (warp == 1) {
-    // ------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
+    } else if (warp == 1) {
+      // ---------------------------------------------------------------- MMA issuer
+      // The whole warp walks the loop and waits on the barriers; one elected lane issues the
+      // tcgen05 instructions (a converged warp + elect.sync compiles to straight-line UTCHMMA).
       constexpr uint32_t idesc_s = umma_idesc_bf16(128, FCP_BQ, 0, 0);    // S^T, dP^T
       constexpr uint32_t idesc_kv = umma_idesc_bf16(128, D, 0, 1);        // dV, dK
       constexpr uint32_t idesc_dq = umma_idesc_bf16(128, FCP_BQ, 1, 1);   // dQ^T
-      const uint32_t k_addr = smem_u32(k_smem), v_addr = smem_u32(v_smem);
-      const uint32_t stage_addr = smem_u32(stage_smem), ds_addr = smem_u32(ds_smem);
+      const uint32_t stage_addr = smem_u32(stage_smem);
+      // descriptors of the item-stationary operands; per-MMA variants only add a byte offset
+      const uint64_t k_kmaj = umma_desc_sw128(smem_u32(k_smem), 16, 1024);            // A of S^T
+      const uint64_t v_kmaj = umma_desc_sw128(smem_u32(v_smem), 16, 1024);            // A of dP^T
+      const uint64_t k_mnmaj = umma_desc_sw128(smem_u32(k_smem), Cfg::kKVPanel, 1024);  // A of dQ^T
+      const uint64_t ds_mnmaj = umma_desc_sw128(smem_u32(ds_smem), 1024, 1024);        // B of dQ^T
       uint32_t n = 0, m = 0;
 
       // S^T(n) = K Q^T  or  dP^T(n) = V dO^T : A = kv tile (K-major), B = q/dO tile (K-major)
-      auto issue_kq = [&](uint32_t d_col, uint32_t a_base, uint32_t b_base) {
+      auto issue_kq = [&](uint32_t d_col, uint64_t a_desc, uint32_t b_base) {
+        const uint64_t b_desc = umma_desc_sw128(b_base, 16, 1024);
 #pragma unroll
         for (int kk = 0; kk < D / 16; ++kk)
           umma_ss(tmem_base + d_col,
-                  umma_desc_sw128(a_base + (kk >> 2) * Cfg::kKVPanel + (kk & 3) * 32, 16, 1024),
-                  umma_desc_sw128(b_base + (kk >> 2) * Cfg::kQPanel + (kk & 3) * 32, 16, 1024),
-                  idesc_s, kk > 0);
+                  umma_desc_add(a_desc, (kk >> 2) * Cfg::kKVPanel + (kk & 3) * 32),
+                  umma_desc_add(b_desc, (kk >> 2) * Cfg::kQPanel + (kk & 3) * 32), idesc_s, kk > 0);
       };
 
       for (int r = 0; r < rounds; ++r) {
@@ -297,23 +347,27 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         {
           const uint32_t st = n % Cfg::kStages;
           mbar_wait(&bars->qdo_full[st], (n / Cfg::kStages) & 1);
-          tc_fence_after();
-          issue_kq(Cfg::kColS + (n & 1) * 64, k_addr, stage_addr + st * Cfg::kStage);
           mbar_wait(&bars->dpt_free, (n & 1) ^ 1);
           tc_fence_after();
-          issue_kq(Cfg::kColDP, v_addr, stage_addr + st * Cfg::kStage + Cfg::kQTile);
-          umma_commit(&bars->st_full);
+          if (elect_one()) {
+            issue_kq(Cfg::kColS + (n & 1) * 64, k_kmaj, stage_addr + st * Cfg::kStage);
+            issue_kq(Cfg::kColDP, v_kmaj, stage_addr + st * Cfg::kStage + Cfg::kQTile);
+            umma_commit(&bars->st_full);
+          }
+          __syncwarp();
         }
         for (int i = 0; i < I; ++i, ++n) {
           if (i + 1 < I) {                       // next iteration's S^T / dP^T run ahead
             const uint32_t n1 = n + 1, st1 = n1 % Cfg::kStages;
             mbar_wait(&bars->qdo_full[st1], (n1 / Cfg::kStages) & 1);
+            mbar_wait(&bars->dpt_free, (n1 & 1) ^ 1);      // softmax(n) holds dP^T(n) in registers
             tc_fence_after();
-            issue_kq(Cfg::kColS + (n1 & 1) * 64, k_addr, stage_addr + st1 * Cfg::kStage);
-            mbar_wait(&bars->dpt_free, (n1 & 1) ^ 1);      // softmax(n) has read dP^T(n)
-            tc_fence_after();
-            issue_kq(Cfg::kColDP, v_addr, stage_addr + st1 * Cfg::kStage + Cfg::kQTile);
-            umma_commit(&bars->st_full);
+            if (elect_one()) {
+              issue_kq(Cfg::kColS + (n1 & 1) * 64, k_kmaj, stage_addr + st1 * Cfg::kStage);
+              issue_kq(Cfg::kColDP, v_kmaj, stage_addr + st1 * Cfg::kStage + Cfg::kQTile);
+              umma_commit(&bars->st_full);
+            }
+            __syncwarp();
           }
           const uint32_t st = n % Cfg::kStages;
           const uint32_t q_base = stage_addr + st * Cfg::kStage, do_base = q_base + Cfg::kQTile;
@@ -322,37 +376,44 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
           if (i == 0) mbar_wait(&bars->dkv_free, (m & 1) ^ 1);
           mbar_wait(&bars->dq_free, (n & 1) ^ 1);
           tc_fence_after();
-          // dV += P^T dO, dK += dS^T Q : A from TMEM, B = dO / Q tile as MN-major [K=q][N=D]
+          if (elect_one()) {
+            // dV += P^T dO, dK += dS^T Q : A from TMEM, B = dO / Q tile as MN-major [K=q][N=D]
+            const uint64_t do_desc = umma_desc_sw128(do_base, Cfg::kQPanel, 1024);
+            const uint64_t q_desc = umma_desc_sw128(q_base, Cfg::kQPanel, 1024);
 #pragma unroll
-          for (int kk = 0; kk < FCP_BQ / 16; ++kk)
-            umma_ts(tmem_base + Cfg::kColDV, tP + kk * 8,
-                    umma_desc_sw128(do_base + kk * 2048, Cfg::kQPanel, 1024), idesc_kv,
-                    (i > 0 || kk > 0) ? 1u : 0u);
+            for (int kk = 0; kk < FCP_BQ / 16; ++kk)
+              umma_ts(tmem_base + Cfg::kColDV, tP + kk * 8, umma_desc_add(do_desc, kk * 2048),
+                      idesc_kv, (i > 0 || kk > 0) ? 1u : 0u);
 #pragma unroll
-          for (int kk = 0; kk < FCP_BQ / 16; ++kk)
-            umma_ts(tmem_base + Cfg::kColDK, tDS + kk * 8,
-                    umma_desc_sw128(q_base + kk * 2048, Cfg::kQPanel, 1024), idesc_kv,
-                    (i > 0 || kk > 0) ? 1u : 0u);
-          // dQ^T = K^T dS^T : A = K tile as MN-major [K=kv][M=d], B = dS^T smem MN-major [K=kv][N=q]
+            for (int kk = 0; kk < FCP_BQ / 16; ++kk)
+              umma_ts(tmem_base + Cfg::kColDK, tDS + kk * 8, umma_desc_add(q_desc, kk * 2048),
+                      idesc_kv, (i > 0 || kk > 0) ? 1u : 0u);
+            // dQ^T = K^T dS^T : A = K tile as MN-major [K=kv][M=d], B = dS^T smem MN-major [K=kv][N=q]
+            const uint64_t ds_desc = umma_desc_add(ds_mnmaj, (n & 1) * Cfg::kDS);
 #pragma unroll
-          for (int kk = 0; kk < 128 / 16; ++kk)
-            umma_ss(tmem_base + Cfg::kColDQ,
-                    umma_desc_sw128(k_addr + kk * 2048, Cfg::kKVPanel, 1024),
-                    umma_desc_sw128(ds_addr + (n & 1) * Cfg::kDS + kk * 2048, 1024, 1024),
-                    idesc_dq, kk > 0);
-          umma_commit(&bars->qdo_free[st]);
-          umma_commit(&bars->ds_free[n & 1]);
-          umma_commit(&bars->dq_full);
+            for (int kk = 0; kk < 128 / 16; ++kk)
+              umma_ss(tmem_base + Cfg::kColDQ, umma_desc_add(k_mnmaj, kk * 2048),
+                      umma_desc_add(ds_desc, kk * 2048), idesc_dq, kk > 0);
+            umma_commit(&bars->qdo_free[st]);
+            umma_commit(&bars->ds_free[n & 1]);
+            umma_commit(&bars->dq_full);
+          }
+          __syncwarp();
         }
-        umma_commit(&bars->dkv_full);
-        umma_commit(&bars->kv_free);
+        if (elect_one()) {
+          umma_commit(&bars->dkv_full);
+          umma_commit(&bars->kv_free);
+        }
+        __syncwarp();
         ++m;
       }
     }
-  } else if (warp >= 4 && warp < 8) {
+  } else if (warp < 8) {
     // ------------------------------------------------------------------ softmax / dS
+    reg_alloc<Cfg::kRegsSoftmax>();
     const int row = (warp & 3) * 32 + lane;            // KV row of the tile = TMEM lane
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
+    const uint32_t stat_base = smem_u32(stat_smem), ds_base = smem_u32(ds_smem) + row * 128;
     uint32_t n = 0, m = 0;
     for (int r = 0; r < rounds; ++r) {
       const int idx = snake_item_b(r, n_items);
@@ -373,56 +434,33 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         continue;
       }
       const int kv_pos = it.kv_pos0 + row;
+      const int warp_kv_max = it.kv_pos0 + (warp & 3) * 32 + 31;
       for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
         const uint32_t st = n % Cfg::kStages;
-        const float2* stat =
-            reinterpret_cast<const float2*>(stage_smem + st * Cfg::kStage + 2 * Cfg::kQTile);
         const uint32_t tS = tmem_base + lane_addr + Cfg::kColS + (n & 1) * 64;
         const uint32_t tDP = tmem_base + lane_addr + Cfg::kColDP;
-        uint8_t* ds_row = ds_smem + (n & 1) * Cfg::kDS + row * 128;
         const int q_pos = w.q_pos();
         // mask needed when some (kv, q) pair of this warp's rows is invisible
-        const bool need_mask = (it.kv_pos0 + (warp & 3) * 32 + 31 > q_pos) || (it.kv_rows < 128);
-        mbar_wait(&bars->qdo_full[st], (n / Cfg::kStages) & 1);   // (lse, delta) of the q tile landed
+        const bool need_mask = (warp_kv_max > q_pos) || (it.kv_rows < 128);
         mbar_wait(&bars->st_full, n & 1);
         tc_fence_after();
-        uint32_t s[2][32];
-        tmem_ld32(tS, s[0]);
-        tmem_ld32(tS + 32, s[1]);
-        mbar_wait(&bars->ds_free[n & 1], ((n >> 1) & 1) ^ 1);   // dQ^T(n-2) has read dS^T smem
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          uint32_t dp[32];
-          tmem_ld32(tDP + h * 32, dp);
-          tmem_ld_wait();
-          if (h == 1) {
-            tc_fence_before();
-            mbar_arrive(&bars->dpt_free);
-          }
-          uint32_t pk_p[16], pk_ds[16];
-#pragma unroll
-          for (int i = 0; i < 32; i += 2) {
-            const float4 st01 = *reinterpret_cast<const float4*>(stat + h * 32 + i);  // lse0,d0,lse1,d1
-            float p0 = fast_exp2(fmaf(__uint_as_float(s[h][i]), scale_log2, -st01.x));
-            float p1 = fast_exp2(fmaf(__uint_as_float(s[h][i + 1]), scale_log2, -st01.z));
-            if (need_mask) {
-              if (!row_valid || kv_pos > q_pos + h * 32 + i) p0 = 0.f;
-              if (!row_valid || kv_pos > q_pos + h * 32 + i + 1) p1 = 0.f;
-            }
-            const float ds0 = p0 * (__uint_as_float(dp[i]) - st01.y);
-            const float ds1 = p1 * (__uint_as_float(dp[i + 1]) - st01.w);
-            pk_p[i >> 1] = pack_bf16(p0, p1);
-            pk_ds[i >> 1] = pack_bf16(ds0, ds1);
-          }
-          tmem_st16(tS + h * 16, pk_p);
-          tmem_st16(tS + 32 + h * 16, pk_ds);
-#pragma unroll
-          for (int c = 0; c < 4; ++c) {                 // 128-byte swizzled row of dS^T
-            const int chunk = (h * 4 + c) ^ (row & 7);
-            *reinterpret_cast<int4*>(ds_row + chunk * 16) =
-                make_int4(pk_ds[4 * c], pk_ds[4 * c + 1], pk_ds[4 * c + 2], pk_ds[4 * c + 3]);
-          }
-        }
+        uint32_t s[64], dp[64];
+        tmem_ld32(tS, *reinterpret_cast<uint32_t(*)[32]>(&s[0]));
+        tmem_ld32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&s[32]));
+        tmem_ld32(tDP, *reinterpret_cast<uint32_t(*)[32]>(&dp[0]));
+        tmem_ld32(tDP + 32, *reinterpret_cast<uint32_t(*)[32]>(&dp[32]));
+        mbar_wait(&bars->qdo_full[st], (n / Cfg::kStages) & 1);   // (lse, delta) of the q tile landed
+        mbar_wait(&bars->ds_free[n & 1], ((n >> 1) & 1) ^ 1);     // dQ^T(n-2) has read dS^T smem
+        tmem_ld_wait();
+        tc_fence_before();
+        mbar_arrive(&bars->dpt_free);                              // dP^T (and S^T) now in registers
+        const uint32_t stat_addr = stat_base + st * Cfg::kStat;
+        const uint32_t ds_row_addr = ds_base + (n & 1) * Cfg::kDS;
+        if (need_mask)
+          bwd_softmax_tile<true>(s, dp, stat_addr, scale_log2, row_valid ? kv_pos - q_pos : FCP_BQ,
+                                 tS, ds_row_addr, row);
+        else
+          bwd_softmax_tile<false>(s, dp, stat_addr, scale_log2, 0, tS, ds_row_addr, row);
         fence_proxy_async_smem();
         tmem_st_wait();
         tc_fence_before();
@@ -465,10 +503,12 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       mbar_arrive(&bars->dkv_free);
       ++m;
     }
-  } else if (warp >= 8) {
+  } else {
     // ------------------------------------------------------------------ dQ drain
+    reg_dealloc<Cfg::kRegsDrain>();
     const int drow = (warp & 3) * 32 + lane;           // d index = TMEM lane of dQ^T
     const uint32_t tDQ = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + Cfg::kColDQ;
+    const uint32_t dq_addr = smem_u32(dq_smem) + drow * 4;
     const bool leader = threadIdx.x == 8 * 32;
     uint32_t n = 0;
     for (int r = 0; r < rounds; ++r) {
@@ -489,7 +529,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         named_bar_sync(1, 128);
         if (drow < D) {
 #pragma unroll
-          for (int q = 0; q < FCP_BQ; ++q) dq_smem[q * D + drow] = __uint_as_float(acc[q >> 5][q & 31]);
+          for (int q = 0; q < FCP_BQ; ++q) sts32(dq_addr + q * D * 4, acc[q >> 5][q & 31]);
         }
         fence_proxy_async_smem();
         named_bar_sync(1, 128);

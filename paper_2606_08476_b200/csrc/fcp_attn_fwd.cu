@@ -133,82 +133,91 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------------ MMA issuer
-    if (lane == 0) {
-      constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
-      constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, 0, 1);
-      const uint32_t q_addr = smem_u32(q_smem), ring_addr = smem_u32(ring);
-      uint32_t kv_n = 0, item_n = 0, p_ph[2] = {0, 0};
+    // The whole warp walks the loop and waits on the barriers; one elected lane issues the
+    // tcgen05 instructions (a converged warp + elect.sync compiles to straight-line UTCHMMA).
+    constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
+    constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, 0, 1);
+    const uint64_t q_desc0 = umma_desc_sw128(smem_u32(q_smem), 16, 1024);          // K-major
+    const uint64_t ring_kmaj = umma_desc_sw128(smem_u32(ring), 16, 1024);          // K tile
+    const uint64_t ring_mnmaj = umma_desc_sw128(smem_u32(ring), Cfg::kPanelBytes, 1024);  // V tile
+    uint32_t kv_n = 0, item_n = 0, p_ph[2] = {0, 0};
 
-      auto issue_qk = [&](int t, uint32_t kslot) {
-        const uint32_t a0 = q_addr + t * Cfg::kTileBytes, b0 = ring_addr + kslot * Cfg::kTileBytes;
+    auto issue_qk = [&](int t, uint32_t kslot) {
+      const uint64_t a0 = umma_desc_add(q_desc0, t * Cfg::kTileBytes);
+      const uint64_t b0 = umma_desc_add(ring_kmaj, kslot * Cfg::kTileBytes);
 #pragma unroll
-        for (int kk = 0; kk < D / 16; ++kk) {
-          const uint32_t off = (kk >> 2) * Cfg::kPanelBytes + (kk & 3) * 32;
-          umma_ss(tmem_base + t * 128, umma_desc_sw128(a0 + off, 16, 1024),
-                  umma_desc_sw128(b0 + off, 16, 1024), idesc_qk, kk > 0);
-        }
-      };
-      auto issue_pv = [&](int t, uint32_t vslot, bool acc) {
-        const uint32_t b0 = ring_addr + vslot * Cfg::kTileBytes;
+      for (int kk = 0; kk < D / 16; ++kk) {
+        const uint32_t off = (kk >> 2) * Cfg::kPanelBytes + (kk & 3) * 32;
+        umma_ss(tmem_base + t * 128, umma_desc_add(a0, off), umma_desc_add(b0, off), idesc_qk,
+                kk > 0);
+      }
+    };
+    auto issue_pv = [&](int t, uint32_t vslot, bool acc) {
+      const uint64_t b0 = umma_desc_add(ring_mnmaj, vslot * Cfg::kTileBytes);
 #pragma unroll
-        for (int kk = 0; kk < 128 / 16; ++kk)
-          umma_ts(tmem_base + (NQ + t) * 128, tmem_base + t * 128 + kk * 8,
-                  umma_desc_sw128(b0 + kk * 2048, Cfg::kPanelBytes, 1024), idesc_pv,
-                  (acc || kk > 0) ? 1u : 0u);
-      };
+      for (int kk = 0; kk < 128 / 16; ++kk)
+        umma_ts(tmem_base + (NQ + t) * 128, tmem_base + t * 128 + kk * 8,
+                umma_desc_add(b0, kk * 2048), idesc_pv, (acc || kk > 0) ? 1u : 0u);
+    };
 
-      for (int r = 0; r < rounds; ++r) {
-        const int idx = snake_item(r, n_items);
-        if (idx < 0) continue;
-        const FwdItem it = items[idx];
-        const int n = it.n_kv_tiles;
-        if (n == 0) continue;
-        mbar_wait(&bars->q_full, item_n & 1);
-        {
-          const uint32_t kslot = kv_n % Cfg::kStages;
-          mbar_wait(&bars->kv_full[kslot], (kv_n / Cfg::kStages) & 1);
-          tc_fence_after();
+    for (int r = 0; r < rounds; ++r) {
+      const int idx = snake_item(r, n_items);
+      if (idx < 0) continue;
+      const FwdItem it = items[idx];
+      const int n = it.n_kv_tiles;
+      if (n == 0) continue;
+      mbar_wait(&bars->q_full, item_n & 1);
+      {
+        const uint32_t kslot = kv_n % Cfg::kStages;
+        mbar_wait(&bars->kv_full[kslot], (kv_n / Cfg::kStages) & 1);
+        tc_fence_after();
+        if (elect_one()) {
           for (int t = 0; t < NQ; ++t) {
             issue_qk(t, kslot);
             umma_commit(&bars->s_full[t]);
           }
           umma_commit(&bars->kv_empty[kslot]);
           if (n == 1) umma_commit(&bars->q_empty);
-          ++kv_n;
         }
-        for (int j = 0; j < n; ++j) {
-          const bool has_next = j + 1 < n;
-          const uint32_t vslot = kv_n % Cfg::kStages, vph = (kv_n / Cfg::kStages) & 1;
-          const uint32_t kslot = (kv_n + 1) % Cfg::kStages,
-                         kph = ((kv_n + 1) / Cfg::kStages) & 1;
-          for (int t = 0; t < NQ; ++t) {
-            mbar_wait(&bars->p_ready[t], p_ph[t]);
-            p_ph[t] ^= 1;
-            if (j == 0) mbar_wait(&bars->o_empty[t], (item_n & 1) ^ 1);
-            if (t == 0) mbar_wait(&bars->kv_full[vslot], vph);
-            tc_fence_after();
+        __syncwarp();
+        ++kv_n;
+      }
+      for (int j = 0; j < n; ++j) {
+        const bool has_next = j + 1 < n;
+        const uint32_t vslot = kv_n % Cfg::kStages, vph = (kv_n / Cfg::kStages) & 1;
+        const uint32_t kslot = (kv_n + 1) % Cfg::kStages,
+                       kph = ((kv_n + 1) / Cfg::kStages) & 1;
+        for (int t = 0; t < NQ; ++t) {
+          mbar_wait(&bars->p_ready[t], p_ph[t]);
+          p_ph[t] ^= 1;
+          if (j == 0) mbar_wait(&bars->o_empty[t], (item_n & 1) ^ 1);
+          if (t == 0) {
+            mbar_wait(&bars->kv_full[vslot], vph);
+            if (has_next) mbar_wait(&bars->kv_full[kslot], kph);
+          }
+          tc_fence_after();
+          if (elect_one()) {
             issue_pv(t, vslot, j > 0);
             if (has_next) {
-              if (t == 0) {
-                mbar_wait(&bars->kv_full[kslot], kph);
-                tc_fence_after();
-              }
               issue_qk(t, kslot);
               umma_commit(&bars->s_full[t]);
             } else {
               umma_commit(&bars->o_full[t]);
             }
           }
+          __syncwarp();
+        }
+        if (elect_one()) {
           umma_commit(&bars->kv_empty[vslot]);
-          ++kv_n;
           if (has_next) {
             umma_commit(&bars->kv_empty[kslot]);
-            ++kv_n;
             if (j + 2 == n) umma_commit(&bars->q_empty);
           }
         }
-        ++item_n;
+        __syncwarp();
+        kv_n += has_next ? 2 : 1;
       }
+      ++item_n;
     }
   } else if (warp >= 4) {
     // ------------------------------------------------------------------ softmax + epilogue

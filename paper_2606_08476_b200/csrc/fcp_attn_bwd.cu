@@ -40,8 +40,13 @@ extern "C" int fcp_debug_trace(long long* out) {
     if (blockIdx.x == 0 && (n) >= 200u && (n) < 264u && (threadIdx.x & 31) == 0)       \
       g_trace[((n) - 200u) * 16 + (id)] = clock64();                                   \
   } while (0)
+#define TRACEV(n, id, v)                                                               \
+  do {                                                                                 \
+    if (blockIdx.x == 0 && (n) >= 200u && (n) < 264u) g_trace[((n) - 200u) * 16 + (id)] = (v); \
+  } while (0)
 #else
 #define TRACE(n, id)
+#define TRACEV(n, id, v)
 #endif
 
 namespace {
@@ -132,7 +137,7 @@ struct BwdCfg {
   // TMEM columns
   static constexpr int kColS = 0, kColDP = 128, kColDQ = 192, kColDV = 256, kColDK = 384;
   // registers per thread after setmaxnreg (launch: 128): control, softmax x2, drain
-  static constexpr int kRegsCtl = 56, kRegsSoftmax = 160, kRegsDrain = 112;
+  static constexpr int kRegsCtl = 96, kRegsSoftmax = 152, kRegsDrain = 104;
   // the MMA thread probes the barriers of its next group before issuing the last kTail MMAs of
   // the current one: the tcgen05 queue holds about 5 MMAs, enough to cover the probe latency
   static constexpr int kTail = 3;
@@ -336,119 +341,116 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       // ---------------------------------------------------------------- MMA issuer
       // One elected thread (elect.sync compiles to straight-line UTCHMMA).  The tcgen05 queue is
       // only about 5 MMAs deep, so issue runs at the pace of execution; the barriers of the next
-      // group are probed (non-blocking) before the last kTail MMAs of the current one, so that
-      // in the steady state the pipe never drains while this thread looks at a barrier.
+      // group are probed (non-blocking) before the last kTail MMAs of the current one, and all
+      // per-iteration scalar work is a handful of 32-bit adds on precomputed descriptor words,
+      // so that in the steady state the pipe never drains between two groups.
       constexpr uint32_t idesc_s = umma_idesc_bf16(128, FCP_BQ, 0, 0);    // S^T, dP^T
       constexpr uint32_t idesc_kv = umma_idesc_bf16(128, D, 0, 1);        // dV, dK
       constexpr uint32_t idesc_dq = umma_idesc_bf16(128, FCP_BQ, 1, 1);   // dQ^T
       constexpr int kTail = Cfg::kTail;
-      const uint32_t stage_addr = smem_u32(stage_smem);
-      // descriptors of the item-stationary operands; per-MMA variants only add a byte offset
-      const uint64_t k_kmaj = umma_desc_sw128(smem_u32(k_smem), 16, 1024);            // A of S^T
-      const uint64_t v_kmaj = umma_desc_sw128(smem_u32(v_smem), 16, 1024);            // A of dP^T
-      const uint64_t k_mnmaj = umma_desc_sw128(smem_u32(k_smem), Cfg::kKVPanel, 1024);  // A of dQ^T
-      const uint64_t ds_mnmaj = umma_desc_sw128(smem_u32(ds_smem), 1024, 1024);        // B of dQ^T
-      uint32_t n = 0, m = 0;
+      constexpr int kSteps = D / 16;
+      // Every operand here uses SWIZZLE_128B with SBO = 1024: the high descriptor word is one
+      // constant, the low word is (address >> 4) | (LBO >> 4) << 16.
+      constexpr uint32_t kHi = (1024u >> 4) | (1u << 14) | (2u << 29);   // SBO, version, swizzle
+      auto lo_word = [](uint32_t saddr, uint32_t lbo) { return ((saddr & 0x3FFFF) >> 4) | ((lbo >> 4) << 16); };
+      auto desc = [](uint32_t lo) { return ((uint64_t)kHi << 32) | lo; };
+      const uint32_t k_kmaj = lo_word(smem_u32(k_smem), 16);                 // A of S^T
+      const uint32_t v_kmaj = lo_word(smem_u32(v_smem), 16);                 // A of dP^T
+      const uint32_t k_mnmaj = lo_word(smem_u32(k_smem), Cfg::kKVPanel);     // A of dQ^T
+      const uint32_t ds_mnmaj = lo_word(smem_u32(ds_smem), 1024);            // B of dQ^T (buffer 0)
+      const uint32_t q_kmaj0 = lo_word(smem_u32(stage_smem), 16);            // B of S^T  (stage 0)
+      const uint32_t q_mnmaj0 = lo_word(smem_u32(stage_smem), Cfg::kQPanel); // B of dK   (stage 0)
+      constexpr uint32_t kStageStep = Cfg::kStage >> 4, kDoStep = Cfg::kQTile >> 4;
+      // ring state of iteration n: stage index, parity of the stage's phase, n & 1
+      uint32_t st = 0, sph = 0, b = 0, mph = 0;
 
-      // S^T(n) = K Q^T  or  dP^T(n) = V dO^T : A = kv tile (K-major), B = q/dO tile (K-major)
-      auto issue_kq = [&](uint32_t d_col, uint64_t a_desc, uint64_t b_desc, int kk0, int kk1) {
+      // S^T = K Q^T  or  dP^T = V dO^T : A = kv tile (K-major), B = q/dO tile (K-major)
+      auto issue_kq = [&](uint32_t d_col, uint32_t a_lo, uint32_t b_lo, int kk0, int kk1) {
 #pragma unroll
         for (int kk = kk0; kk < kk1; ++kk)
           umma_ss(tmem_base + d_col,
-                  umma_desc_add(a_desc, (kk >> 2) * Cfg::kKVPanel + (kk & 3) * 32),
-                  umma_desc_add(b_desc, (kk >> 2) * Cfg::kQPanel + (kk & 3) * 32), idesc_s, kk > 0);
+                  desc(a_lo + (((kk >> 2) * Cfg::kKVPanel + (kk & 3) * 32) >> 4)),
+                  desc(b_lo + (((kk >> 2) * Cfg::kQPanel + (kk & 3) * 32) >> 4)), idesc_s, kk > 0);
       };
-      constexpr int kSteps = D / 16;
 
       for (int r = 0; r < rounds; ++r) {
         const int idx = snake_item_b(r, n_items);
         if (idx < 0) continue;
-        const BwdItem it = items[idx];
-        const int I = it.n_iters;
+        const int I = items[idx].n_iters;
         if (I == 0) continue;
-        mbar_wait(&bars->kv_full, m & 1);
+        mbar_wait(&bars->kv_full, mph);
         // prologue: S^T and dP^T of the item's first iteration
         {
-          const uint32_t st = n % Cfg::kStages;
-          mbar_wait(&bars->qdo_full[st], (n / Cfg::kStages) & 1);
-          mbar_wait(&bars->dpt_free, (n & 1) ^ 1);
+          mbar_wait(&bars->qdo_full[st], sph);
+          mbar_wait(&bars->dpt_free, b ^ 1);
           tc_fence_after();
-          const uint64_t q_desc = umma_desc_sw128(stage_addr + st * Cfg::kStage, 16, 1024);
-          issue_kq(Cfg::kColS + (n & 1) * 64, k_kmaj, q_desc, 0, kSteps);
-          issue_kq(Cfg::kColDP, v_kmaj, umma_desc_add(q_desc, Cfg::kQTile), 0, kSteps);
+          const uint32_t q_lo = q_kmaj0 + st * kStageStep;
+          issue_kq(Cfg::kColS + b * 64, k_kmaj, q_lo, 0, kSteps);
+          issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, 0, kSteps);
           umma_commit(&bars->st_full);
         }
         bool ok_a = false;                       // barriers of the next S^T/dP^T group already seen
-        for (int i = 0; i < I; ++i, ++n) {
+        for (int i = 0; i < I; ++i) {
+          // ring state of iterations n+1 and n+2
+          const uint32_t st1 = st + 1 == Cfg::kStages ? 0 : st + 1, sph1 = st + 1 == Cfg::kStages ? sph ^ 1 : sph;
+          const uint32_t st2 = st1 + 1 == Cfg::kStages ? 0 : st1 + 1, sph2 = st1 + 1 == Cfg::kStages ? sph1 ^ 1 : sph1;
           bool ok_b = false;                     // barriers of this iteration's dV/dK/dQ group seen
           if (i + 1 < I) {                       // next iteration's S^T / dP^T run ahead
-            const uint32_t n1 = n + 1, st1 = n1 % Cfg::kStages;
             if (!ok_a) {
-              mbar_wait(&bars->qdo_full[st1], (n1 / Cfg::kStages) & 1);
-              mbar_wait(&bars->dpt_free, (n1 & 1) ^ 1);    // softmax(n) holds dP^T(n) in registers
+              mbar_wait(&bars->qdo_full[st1], sph1);
+              mbar_wait(&bars->dpt_free, b);     // softmax(n) holds dP^T(n) in registers
             }
             tc_fence_after();
-            const uint64_t q_desc = umma_desc_sw128(stage_addr + st1 * Cfg::kStage, 16, 1024);
-            issue_kq(Cfg::kColS + (n1 & 1) * 64, k_kmaj, q_desc, 0, kSteps);
-            issue_kq(Cfg::kColDP, v_kmaj, umma_desc_add(q_desc, Cfg::kQTile), 0, kSteps - kTail);
-            ok_b = mbar_test(&bars->p_ready, n & 1) & mbar_test(&bars->dq_free, (n & 1) ^ 1) &
-                   (i > 0 || mbar_test(&bars->dkv_free, (m & 1) ^ 1));
-#ifdef FCP_EXP_NOPROBE_B
-            ok_b = false;
-#endif
-            issue_kq(Cfg::kColDP, v_kmaj, umma_desc_add(q_desc, Cfg::kQTile), kSteps - kTail, kSteps);
+            const uint32_t q_lo = q_kmaj0 + st1 * kStageStep;
+            issue_kq(Cfg::kColS + (b ^ 1) * 64, k_kmaj, q_lo, 0, kSteps);
+            issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, 0, kSteps - kTail);
+            ok_b = mbar_test(&bars->p_ready, b) & mbar_test(&bars->dq_free, b ^ 1) &
+                   (i > 0 || mbar_test(&bars->dkv_free, mph ^ 1));
+            issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, kSteps - kTail, kSteps);
             umma_commit(&bars->st_full);
           }
-          const uint32_t st = n % Cfg::kStages;
-          const uint32_t q_base = stage_addr + st * Cfg::kStage, do_base = q_base + Cfg::kQTile;
-          // P^T / dS^T of q columns [32h, 32h+32) live in columns [32h, 32h+16) / [32h+16, 32h+32)
-          // of the S^T buffer: each softmax warpgroup overwrites only the columns it has loaded
-          const uint32_t tP = tmem_base + Cfg::kColS + (n & 1) * 64, tDS = tP + 16;
           if (!ok_b) {
-            mbar_wait(&bars->p_ready, n & 1);
-            if (i == 0) mbar_wait(&bars->dkv_free, (m & 1) ^ 1);
-            mbar_wait(&bars->dq_free, (n & 1) ^ 1);
+            mbar_wait(&bars->p_ready, b);
+            if (i == 0) mbar_wait(&bars->dkv_free, mph ^ 1);
+            mbar_wait(&bars->dq_free, b ^ 1);
           }
           tc_fence_after();
+          // P^T / dS^T of q columns [32h, 32h+32) live in columns [32h, 32h+16) / [32h+16, 32h+32)
+          // of the S^T buffer: each softmax warpgroup overwrites only the columns it has loaded
+          const uint32_t tP = tmem_base + Cfg::kColS + b * 64, tDS = tP + 16;
           // dV += P^T dO, dK += dS^T Q : A from TMEM, B = dO / Q tile as MN-major [K=q][N=D]
-          const uint64_t do_desc = umma_desc_sw128(do_base, Cfg::kQPanel, 1024);
-          const uint64_t q_desc = umma_desc_sw128(q_base, Cfg::kQPanel, 1024);
+          const uint32_t q_lo = q_mnmaj0 + st * kStageStep, do_lo = q_lo + kDoStep;
 #pragma unroll
           for (int kk = 0; kk < FCP_BQ / 16; ++kk)
             umma_ts(tmem_base + Cfg::kColDV, tP + (kk >> 1) * 32 + (kk & 1) * 8,
-                    umma_desc_add(do_desc, kk * 2048),
-                    idesc_kv, (i > 0 || kk > 0) ? 1u : 0u);
+                    desc(do_lo + kk * (2048 >> 4)), idesc_kv, (i > 0 || kk > 0) ? 1u : 0u);
 #pragma unroll
           for (int kk = 0; kk < FCP_BQ / 16; ++kk)
             umma_ts(tmem_base + Cfg::kColDK, tDS + (kk >> 1) * 32 + (kk & 1) * 8,
-                    umma_desc_add(q_desc, kk * 2048),
-                    idesc_kv, (i > 0 || kk > 0) ? 1u : 0u);
+                    desc(q_lo + kk * (2048 >> 4)), idesc_kv, (i > 0 || kk > 0) ? 1u : 0u);
           // dQ^T = K^T dS^T : A = K tile as MN-major [K=kv][M=d], B = dS^T smem MN-major [K=kv][N=q]
-          const uint64_t ds_desc = umma_desc_add(ds_mnmaj, (n & 1) * Cfg::kDS);
+          const uint32_t ds_lo = ds_mnmaj + b * (Cfg::kDS >> 4);
 #pragma unroll
           for (int kk = 0; kk < 8 - kTail; ++kk)
-            umma_ss(tmem_base + Cfg::kColDQ, umma_desc_add(k_mnmaj, kk * 2048),
-                    umma_desc_add(ds_desc, kk * 2048), idesc_dq, kk > 0);
+            umma_ss(tmem_base + Cfg::kColDQ, desc(k_mnmaj + kk * (2048 >> 4)),
+                    desc(ds_lo + kk * (2048 >> 4)), idesc_dq, kk > 0);
           ok_a = false;
-          if (i + 2 < I) {
-            const uint32_t n2 = n + 2, st2 = n2 % Cfg::kStages;
-            ok_a = mbar_test(&bars->qdo_full[st2], (n2 / Cfg::kStages) & 1) &
-                   mbar_test(&bars->dpt_free, (n2 & 1) ^ 1);
-#ifdef FCP_EXP_NOPROBE_A
-            ok_a = false;
-#endif
-          }
+          if (i + 2 < I)
+            ok_a = mbar_test(&bars->qdo_full[st2], sph2) & mbar_test(&bars->dpt_free, b ^ 1);
 #pragma unroll
           for (int kk = 8 - kTail; kk < 8; ++kk)
-            umma_ss(tmem_base + Cfg::kColDQ, umma_desc_add(k_mnmaj, kk * 2048),
-                    umma_desc_add(ds_desc, kk * 2048), idesc_dq, 1u);
+            umma_ss(tmem_base + Cfg::kColDQ, desc(k_mnmaj + kk * (2048 >> 4)),
+                    desc(ds_lo + kk * (2048 >> 4)), idesc_dq, 1u);
           umma_commit(&bars->qdo_free[st]);
-          umma_commit(&bars->ds_free[n & 1]);
+          umma_commit(&bars->ds_free[b]);
           umma_commit(&bars->dq_full);
+          st = st1;
+          sph = sph1;
+          b ^= 1;
         }
         umma_commit(&bars->dkv_full);
         umma_commit(&bars->kv_free);
-        ++m;
+        mph ^= 1;
       }
     }
   } else if (warp < 12) {

@@ -155,12 +155,6 @@ struct BwdBarriers {
 };
 static_assert(sizeof(BwdBarriers) <= 256, "barrier block");
 
-__device__ __forceinline__ int snake_item_b(int round, int n_items) {
-  const int g = gridDim.x, b = blockIdx.x;
-  const int idx = round * g + ((round & 1) ? (g - 1 - b) : b);
-  return idx < n_items ? idx : -1;
-}
-
 // Enumerates the inner iterations of an item in the one order every warp role follows:
 // shards seen by the KV tile -> 64-row q tiles -> the G query heads of the kv head.
 struct IterWalk {
@@ -254,7 +248,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_do,
                   const __grid_constant__ CUtensorMap tmap_k,
                   const __grid_constant__ CUtensorMap tmap_v,
-                  const BwdItem* __restrict__ items, int n_items,
+                  const BwdItem* __restrict__ items, const int32_t* __restrict__ cta_off,
                   const BwdSub* __restrict__ subs, const float2* __restrict__ lsed,
                   float* __restrict__ dq_acc, void* __restrict__ dk_out,
                   void* __restrict__ dv_out, int dkv_f32, int64_t n_q_pad, int Hkv, int G,
@@ -296,7 +290,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
-  const int rounds = (n_items + gridDim.x - 1) / gridDim.x;
+  const int item_begin = cta_off[blockIdx.x], item_end = cta_off[blockIdx.x + 1];   // this CTA's work list
 
   if (warp < 4) {
     reg_dealloc<Cfg::kRegsCtl>();
@@ -307,9 +301,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       prefetch_tmap(&tmap_k);
       prefetch_tmap(&tmap_v);
       uint32_t n = 0, m = 0;          // global iteration / item counters
-      for (int r = 0; r < rounds; ++r) {
-        const int idx = snake_item_b(r, n_items);
-        if (idx < 0) continue;
+      for (int idx = item_begin; idx < item_end; ++idx) {
         const BwdItem it = items[idx];
         if (it.n_iters == 0) continue;
         mbar_wait(&bars->kv_free, (m & 1) ^ 1);
@@ -373,9 +365,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
                   desc(b_lo + (((kk >> 2) * Cfg::kQPanel + (kk & 3) * 32) >> 4)), idesc_s, kk > 0);
       };
 
-      for (int r = 0; r < rounds; ++r) {
-        const int idx = snake_item_b(r, n_items);
-        if (idx < 0) continue;
+      for (int idx = item_begin; idx < item_end; ++idx) {
         const int I = items[idx].n_iters;
         if (I == 0) continue;
         mbar_wait(&bars->kv_full, mph);
@@ -465,9 +455,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t stat_base = smem_u32(stat_smem) + half * 32 * 8;
     const uint32_t ds_base = smem_u32(ds_smem) + row * 128;
     uint32_t n = 0, m = 0;
-    for (int r = 0; r < rounds; ++r) {
-      const int idx = snake_item_b(r, n_items);
-      if (idx < 0) continue;
+    for (int idx = item_begin; idx < item_end; ++idx) {
       const BwdItem it = items[idx];
       const bool row_valid = row < it.kv_rows;
       // output row of this thread (half 0 writes dv, half 1 writes dk), bf16 or fp32 elements
@@ -558,9 +546,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t dq_addr = smem_u32(dq_smem) + drow * 4;
     const bool leader = threadIdx.x == 12 * 32;
     uint32_t n = 0;
-    for (int r = 0; r < rounds; ++r) {
-      const int idx = snake_item_b(r, n_items);
-      if (idx < 0) continue;
+    for (int idx = item_begin; idx < item_end; ++idx) {
       const BwdItem it = items[idx];
       if (it.n_iters == 0) continue;
       for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
@@ -633,11 +619,12 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              Cfg::kSmemBytes) != cudaSuccess)
       return FCP_CUDA;
-    const int grid = std::min(n_items, num_sms());
+    const int grid = s->n_cta;
     if (a->ev_start && cudaEventRecord((cudaEvent_t)a->ev_start, st) != cudaSuccess)
       return FCP_CUDA;
     kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(
-        mq, mdo, mk, mv, reinterpret_cast<const BwdItem*>(ws + s->off_bwd), n_items,
+        mq, mdo, mk, mv, reinterpret_cast<const BwdItem*>(ws + s->off_bwd),
+        reinterpret_cast<const int32_t*>(ws + s->off_bwd_cta),
         reinterpret_cast<const BwdSub*>(ws + s->off_sub), lsed, dq_acc, dk, dv,
         a->dkv_dtype == FCP_DTYPE_F32, s->n_q_pad, s->Hkv, s->G, a->scale, a->scale * kLog2e);
     if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;

@@ -46,23 +46,12 @@ struct FwdBarriers {
   uint32_t tmem_base;
 };
 
-// Static cost-balanced assignment: the list is sorted by descending cost; rounds of gridDim.x
-// items are dealt out alternately forwards and backwards (snake order).
-__device__ __forceinline__ int snake_item(int round, int n_items) {
-  const int g = gridDim.x, b = blockIdx.x;
-  const int idx = round * g + ((round & 1) ? (g - 1 - b) : b);
-  return idx < n_items ? idx : -1;
-}
-__device__ __forceinline__ int snake_rounds(int n_items) {
-  return (n_items + gridDim.x - 1) / gridDim.x;
-}
-
 template <int D, int NQ>
 __global__ void __launch_bounds__(FwdCfg<D, NQ>::kThreads, 1)
 fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v,
-                    const FwdItem* __restrict__ items, int n_items,
+                    const FwdItem* __restrict__ items, const int32_t* __restrict__ cta_off,
                     __nv_bfloat16* __restrict__ o, float* __restrict__ lse,
                     int64_t n_q, int Hq, float scale_log2) {
   using Cfg = FwdCfg<D, NQ>;
@@ -96,7 +85,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
-  const int rounds = snake_rounds(n_items);
+  const int item_begin = cta_off[blockIdx.x], item_end = cta_off[blockIdx.x + 1];   // this CTA's work list
 
   if (warp == 0) {
     // ------------------------------------------------------------------ TMA producer
@@ -105,9 +94,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       prefetch_tmap(&tmap_k);
       prefetch_tmap(&tmap_v);
       uint32_t kv_n = 0, item_n = 0;
-      for (int r = 0; r < rounds; ++r) {
-        const int idx = snake_item(r, n_items);
-        if (idx < 0) continue;
+      for (int idx = item_begin; idx < item_end; ++idx) {
         const FwdItem it = items[idx];
         if (it.n_kv_tiles == 0) continue;
         mbar_wait(&bars->q_empty, (item_n & 1) ^ 1);
@@ -160,9 +147,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
                 umma_desc_add(b0, kk * 2048), idesc_pv, (acc || kk > 0) ? 1u : 0u);
     };
 
-    for (int r = 0; r < rounds; ++r) {
-      const int idx = snake_item(r, n_items);
-      if (idx < 0) continue;
+    for (int idx = item_begin; idx < item_end; ++idx) {
       const FwdItem it = items[idx];
       const int n = it.n_kv_tiles;
       if (n == 0) continue;
@@ -228,9 +213,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t tO = tmem_base + lane_addr + (NQ + t) * 128;
     uint32_t s_ph = 0, o_ph = 0;
 
-    for (int r = 0; r < rounds; ++r) {
-      const int idx = snake_item(r, n_items);
-      if (idx < 0) continue;
+    for (int idx = item_begin; idx < item_end; ++idx) {
       const FwdItem it = items[idx];
       const int n = it.n_kv_tiles;
       const int head = it.head0 + t;
@@ -357,15 +340,15 @@ int launch_fwd(const fcp_attn_args* a, const fcp_sched* s) {
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes) !=
       cudaSuccess)
     return FCP_CUDA;
-  const int n_items = (int)s->fwd.size();
-  const int grid = std::min(n_items, num_sms());
+  const int grid = s->n_cta;
   const FwdItem* items =
       reinterpret_cast<const FwdItem*>(static_cast<const char*>(a->workspace) + s->off_fwd);
   cudaStream_t st = (cudaStream_t)a->stream;
   if (a->ev_start && cudaEventRecord((cudaEvent_t)a->ev_start, st) != cudaSuccess) return FCP_CUDA;
   kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(
-      mq, mk, mv, items, n_items, static_cast<__nv_bfloat16*>(a->o), a->lse, s->n_q, s->Hq,
-      a->scale * kLog2e);
+      mq, mk, mv, items,
+      reinterpret_cast<const int32_t*>(static_cast<const char*>(a->workspace) + s->off_fwd_cta),
+      static_cast<__nv_bfloat16*>(a->o), a->lse, s->n_q, s->Hq, a->scale * kLog2e);
   if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
   if (a->ev_stop && cudaEventRecord((cudaEvent_t)a->ev_stop, st) != cudaSuccess) return FCP_CUDA;
   return FCP_OK;

@@ -246,6 +246,8 @@ extern "C" int fcp_sched_upload(const fcp_sched* s, void* workspace, void* strea
   ok = ok && put(s->off_fwd, s->fwd.data(), s->fwd.size() * sizeof(FwdItem));
   ok = ok && put(s->off_bwd, s->bwd.data(), s->bwd.size() * sizeof(BwdItem));
   ok = ok && put(s->off_sub, s->bwd_sub.data(), s->bwd_sub.size() * sizeof(BwdSub));
+  ok = ok && put(s->off_fwd_cta, s->fwd_cta_off.data(), s->fwd_cta_off.size() * sizeof(int32_t));
+  ok = ok && put(s->off_bwd_cta, s->bwd_cta_off.data(), s->bwd_cta_off.size() * sizeof(int32_t));
   ok = ok && put(s->off_shard_meta, s->tile_meta.data(), s->tile_meta.size() * sizeof(int32_t));
   // The sources are pageable host vectors owned by the schedule: cudaMemcpyAsync returns once
   // they are staged, so no synchronisation is needed here.

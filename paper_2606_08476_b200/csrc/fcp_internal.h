@@ -68,12 +68,16 @@ struct fcp_sched {
   std::vector<int32_t> cu_q, q_pos_off, shard_seg, cu_k;
   std::vector<int32_t> shard_pad0;                 // [ns] first padded row of each shard
   std::vector<int32_t> tile_meta;                  // per padded 64-row tile: (local row0, valid rows)
+  // Work lists, grouped by CTA: CTA c of the persistent grid walks fwd[fwd_cta_off[c] ..
+  // fwd_cta_off[c+1]) in order (greedy longest-processing-time assignment, fcp_sched.cpp).
+  int32_t n_cta = 0;
   std::vector<FwdItem> fwd;
   std::vector<BwdItem> bwd;
+  std::vector<int32_t> fwd_cta_off, bwd_cta_off;   // [n_cta + 1]
   std::vector<BwdSub> bwd_sub;
   int64_t fwd_kv_tiles = 0, bwd_tile_pairs = 0;
   uint64_t useful_pairs = 0;
   // workspace layout (byte offsets, 256-byte aligned)
   size_t off_counters = 0, off_fwd = 0, off_bwd = 0, off_sub = 0, off_shard_meta = 0,
-         off_lsed = 0, off_dq = 0, total = 0;
+         off_fwd_cta = 0, off_bwd_cta = 0, off_lsed = 0, off_dq = 0, total = 0;
 };

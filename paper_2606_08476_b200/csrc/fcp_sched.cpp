@@ -1,15 +1,53 @@
 // Tile schedule of one rank (host part): enumerates the forward (shard, q-tile, head-pack) and
 // backward (segment, kv-tile, kv-head) work items, skips fully masked tiles and orders items by
-// descending cost so that short shards do not starve the SMs (short shards
-// lower kernel efficiency).  The device kernels pull items from these lists with an atomic
-// counter (persistent CTAs).
+// descending cost and assigns them to the persistent CTAs by greedy longest-processing-time, so
+// that short shards do not starve the SMs (short shards lower kernel
+// efficiency).  The assignment is static and deterministic; every CTA walks its own list.
+#include <cuda_runtime.h>
+
 #include <algorithm>
 #include <new>
+#include <queue>
 
 #include "fcp_internal.h"
 
 namespace {
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Persistent grid size = SM count of the current device (148 on B200; also the value used when
+// no device is visible, e.g. when a schedule is built on a CPU-only box).
+int32_t grid_ctas() {
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess ||
+      cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
+    cudaGetLastError();
+    return 148;
+  }
+  return n;
+}
+
+// Greedy longest-processing-time assignment of items (already sorted by descending cost) to
+// n_cta persistent CTAs; `items` is permuted so that every CTA's list is contiguous and
+// cta_off[c] .. cta_off[c+1] delimits it.  Deterministic: ties go to the lowest CTA index.
+template <typename Item, typename Cost>
+void assign_lpt(std::vector<Item>& items, int32_t n_cta, Cost cost, std::vector<int32_t>& cta_off) {
+  typedef std::pair<int64_t, int32_t> Load;      // (load, cta)
+  std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
+  for (int32_t c = 0; c < n_cta; ++c) heap.push(Load(0, c));
+  std::vector<std::vector<Item>> bins(n_cta);
+  for (const Item& it : items) {
+    Load l = heap.top();
+    heap.pop();
+    bins[l.second].push_back(it);
+    heap.push(Load(l.first + cost(it), l.second));
+  }
+  cta_off.assign(n_cta + 1, 0);
+  size_t k = 0;
+  for (int32_t c = 0; c < n_cta; ++c) {
+    for (const Item& it : bins[c]) items[k++] = it;
+    cta_off[c + 1] = (int32_t)k;
+  }
+}
 }
 
 extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
@@ -81,6 +119,10 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
   }
   std::stable_sort(s->fwd.begin(), s->fwd.end(),
                    [](const FwdItem& x, const FwdItem& y) { return x.n_kv_tiles > y.n_kv_tiles; });
+  s->n_cta = grid_ctas();
+  // cost in KV-tile steps; +1 for the per-item Q load and epilogue
+  assign_lpt(s->fwd, s->n_cta, [](const FwdItem& x) { return (int64_t)x.n_kv_tiles + 1; },
+             s->fwd_cta_off);
 
   // ---- backward items ----
   std::vector<std::vector<int32_t>> seg_shards(n_segs);
@@ -120,6 +162,9 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
   }
   std::stable_sort(s->bwd.begin(), s->bwd.end(),
                    [](const BwdItem& x, const BwdItem& y) { return x.n_iters > y.n_iters; });
+  // cost in inner iterations; +2 for the per-item K/V load and the dK/dV epilogue
+  assign_lpt(s->bwd, s->n_cta, [](const BwdItem& x) { return (int64_t)x.n_iters + 2; },
+             s->bwd_cta_off);
 
   // ---- workspace layout ----
   size_t o = 0;
@@ -127,6 +172,8 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
   s->off_fwd = o;       o = align_up(o + s->fwd.size() * sizeof(FwdItem), 256);
   s->off_bwd = o;       o = align_up(o + s->bwd.size() * sizeof(BwdItem), 256);
   s->off_sub = o;       o = align_up(o + s->bwd_sub.size() * sizeof(BwdSub), 256);
+  s->off_fwd_cta = o;   o = align_up(o + s->fwd_cta_off.size() * sizeof(int32_t), 256);
+  s->off_bwd_cta = o;   o = align_up(o + s->bwd_cta_off.size() * sizeof(int32_t), 256);
   s->off_shard_meta = o;  // per padded 64-row tile: (local row0, valid rows)
   o = align_up(o + (size_t)(s->n_q_pad / FCP_BQ) * 2 * sizeof(int32_t), 256);
   s->off_lsed = o;      o = align_up(o + (size_t)s->Hq * s->n_q_pad * 2 * sizeof(float), 256);

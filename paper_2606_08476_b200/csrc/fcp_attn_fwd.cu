@@ -2,21 +2,24 @@
 //
 // One persistent CTA per SM.  A work item is one 128-row q tile of one shard for a pack of NQ
 // query heads that share a kv head (GQA): the NQ tiles share every K/V tile staged in shared
-// memory and ping-pong on the tensor core — while the softmax warps of one tile work, the
-// MMAs of the other tile run.
+// memory.  The pipeline keeps the tensor pipe and the MUFU busy at the same time:
+//   S_t(j+1) = Q_t K_{j+1}^T is issued as soon as the softmax of tile j has LOADED S_t(j) into
+//   registers (P does not alias S: it goes through shared memory), so the softmax warps run
+//   back to back and O_t += P_t(j) V_j only has to keep up.
 //
-//   warp 0      TMA producer   Q (once per item), K/V tiles through a ring of smem stages
-//   warp 1      MMA issuer     one elected thread: S_t = Q_t K^T (SS), O_t += P_t V (A = P from
-//                              TMEM, B = V MN-major); it probes the next group's barriers before
-//                              the last MMAs of the current group (the tcgen05 queue is ~5 deep)
+//   warp 0      TMA producer   Q (once per item); K/V tiles through a 3-slot ring in the order
+//                              the MMAs consume them: K0, K1, V0, K2, V1, ...
+//   warp 1      MMA issuer     one elected thread; per KV tile j: S_t(j+1) (SS), then
+//                              O_t += P_t(j) V_j (SS: A = P in swizzled smem, B = V MN-major);
+//                              it probes the next group's barriers before the last MMAs of the
+//                              current group (the tcgen05 queue is ~5 deep)
 //   warps 4..   softmax        one warpgroup per q tile, one query row per thread: mask from
-//                              (q_pos0 + row, kv_len), online softmax in the log2 domain whose
-//                              fast path exponentiates against the running max of the earlier
-//                              tiles (no max -> exp dependency) and rescales O only when a row
-//                              grew by more than 2^8; P written back to TMEM as bf16 over S,
-//                              epilogue o = O / l
+//                              (q_pos0 + row, kv_len), online softmax in the log2 domain that
+//                              exponentiates against the running max of the earlier tiles (no
+//                              max -> exp dependency) and rescales O only when a row grew by
+//                              more than 2^8; bf16 P into shared memory; epilogue o = O / l
 //
-// TMEM columns: S_t at 128 t, O_t at 128 (NQ + t); P_t aliases the first 64 columns of S_t.
+// TMEM columns: S_t at 128 t, O_t at 128 (NQ + t).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -51,33 +54,35 @@ struct FwdCfg {
   static constexpr int kTileBytes = 128 * D * 2;           // one Q, K or V tile
   static constexpr int kPanelBytes = 128 * 128;            // 128 rows x 64 bf16
   static constexpr int kPanels = D / 64;
-  static constexpr int kStages = (D == 128) ? 4 : 6;       // ring slots, each one K or V tile
-  // softmax warpgroups per q tile: each takes 128 / kHalves key columns of every KV tile.
-  // MUFU (16 ex2/clk/SM) bounds the softmax of a 128x128 tile at 1024 clocks whatever the warp
-  // count, so one warpgroup per tile (no cross-warpgroup exchange) is the faster layout.
-  static constexpr int kHalves = 1;
-  static constexpr int kSoftmaxThreads = 128 * kHalves;    // per q tile
-  static constexpr int kThreads = 128 + kSoftmaxThreads * NQ;
+  static constexpr int kPBytes = 128 * 128 * 2;            // bf16 P of one q tile: 2 panels
+  static constexpr int kStages = (D == 128) ? 3 : 6;       // ring slots, each one K or V tile
+  static constexpr int kThreads = 128 + 128 * NQ;
   static constexpr int kTmemCols = 256 * NQ;
-  static constexpr int kSmemData = (NQ + kStages) * kTileBytes;
-  static constexpr int kXchBytes = NQ * 2 * 128 * 4;       // row max / row sum exchange (kHalves = 2)
-  static constexpr int kSmemBytes = 1024 + kSmemData + kXchBytes + 1024;
+  static constexpr int kOffP = NQ * kTileBytes;
+  static constexpr int kOffRing = kOffP + NQ * kPBytes;
+  static constexpr int kSmemData = kOffRing + kStages * kTileBytes;
+  static constexpr int kSmemBytes = 1024 + kSmemData + 256;
   // registers per thread after setmaxnreg (multiples of 8).  The CTA owns (launch registers x
   // threads): the sum over its warpgroups must stay below.
   static constexpr int kLaunchRegs = (65536 / kThreads) / 8 * 8 > 255 ? 248 : (65536 / kThreads) / 8 * 8;
-  static constexpr int kRegsCtl = 80;
-  static constexpr int kRegsSoftmaxRaw =
-      (kLaunchRegs * (kThreads / 128) - kRegsCtl) / (kHalves * NQ) / 8 * 8;
+  static constexpr int kRegsCtl = 72;
+  static constexpr int kRegsSoftmaxRaw = (kLaunchRegs * (kThreads / 128) - kRegsCtl) / NQ / 8 * 8;
   static constexpr int kRegsSoftmax = kRegsSoftmaxRaw > 232 ? 232 : kRegsSoftmaxRaw;
   static constexpr int kTail = 3;   // MMAs issued after the probe of the next group's barriers
 };
+static_assert(FwdCfg<128, 2>::kSmemBytes <= 232448, "fwd shared memory exceeds 227 KB");
 
 struct FwdBarriers {
   uint64_t q_full, q_empty;
   uint64_t kv_full[8], kv_empty[8];
-  uint64_t s_full[2], p_ready[2], o_full[2], o_empty[2];
+  uint64_t s_full[2];    // S_t written by the MMAs               -> softmax
+  uint64_t s_free[2];    // softmax holds S_t in registers         -> MMA may overwrite S_t
+  uint64_t p_ready[2];   // P_t in shared memory, O_t rescaled     -> MMA
+  uint64_t pv_done[2];   // O_t += P_t V complete: P_t smem free, O_t stable (last tile: final)
+  uint64_t o_empty[2];   // epilogue has read O_t                  -> MMA may overwrite O_t
   uint32_t tmem_base;
 };
+static_assert(sizeof(FwdBarriers) <= 256, "barrier block");
 
 template <int D, int NQ>
 __global__ void __launch_bounds__(FwdCfg<D, NQ>::kThreads, 1)
@@ -92,9 +97,9 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
                                              ~uintptr_t(1023));
   uint8_t* q_smem = smem;                                  // NQ tiles
-  uint8_t* ring = smem + NQ * Cfg::kTileBytes;             // kStages tiles
-  float* xch = reinterpret_cast<float*>(smem + Cfg::kSmemData);   // [NQ][2 halves][128 rows]
-  FwdBarriers* bars = reinterpret_cast<FwdBarriers*>(smem + Cfg::kSmemData + Cfg::kXchBytes);
+  uint8_t* p_smem = smem + Cfg::kOffP;                     // NQ tiles of bf16 P
+  uint8_t* ring = smem + Cfg::kOffRing;                    // kStages tiles
+  FwdBarriers* bars = reinterpret_cast<FwdBarriers*>(smem + Cfg::kSmemData);
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
@@ -108,9 +113,10 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     }
     for (int t = 0; t < NQ; ++t) {
       mbar_init(&bars->s_full[t], 1);
-      mbar_init(&bars->p_ready[t], Cfg::kSoftmaxThreads);
-      mbar_init(&bars->o_full[t], 1);
-      mbar_init(&bars->o_empty[t], Cfg::kSoftmaxThreads);
+      mbar_init(&bars->s_free[t], 128);
+      mbar_init(&bars->p_ready[t], 128);
+      mbar_init(&bars->pv_done[t], 1);
+      mbar_init(&bars->o_empty[t], 128);
     }
     fence_barrier_init();
   }
@@ -128,36 +134,40 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       prefetch_tmap(&tmap_q);
       prefetch_tmap(&tmap_k);
       prefetch_tmap(&tmap_v);
-      uint32_t kv_n = 0, item_n = 0;
+      uint32_t slot = 0, sph = 0, iph = 0;
+      auto load_kv = [&](const CUtensorMap* tm, int kv_head, int row0) {
+        mbar_wait(&bars->kv_empty[slot], sph ^ 1);
+        mbar_arrive_expect_tx(&bars->kv_full[slot], Cfg::kTileBytes);
+        for (int pn = 0; pn < Cfg::kPanels; ++pn)
+          tma_load_3d(ring + slot * Cfg::kTileBytes + pn * Cfg::kPanelBytes, tm,
+                      &bars->kv_full[slot], pn * 64, kv_head, row0);
+        if (++slot == (uint32_t)Cfg::kStages) { slot = 0; sph ^= 1; }
+      };
       for (int idx = item_begin; idx < item_end; ++idx) {
         const FwdItem it = items[idx];
-        if (it.n_kv_tiles == 0) continue;
-        mbar_wait(&bars->q_empty, (item_n & 1) ^ 1);
+        const int n = it.n_kv_tiles;
+        if (n == 0) continue;
+        mbar_wait(&bars->q_empty, iph ^ 1);
         mbar_arrive_expect_tx(&bars->q_full, NQ * Cfg::kTileBytes);
         for (int t = 0; t < NQ; ++t)
           for (int pn = 0; pn < Cfg::kPanels; ++pn)
             tma_load_3d(q_smem + t * Cfg::kTileBytes + pn * Cfg::kPanelBytes, &tmap_q,
                         &bars->q_full, pn * 64, it.head0 + t, it.q_row0);
-        for (int j = 0; j < it.n_kv_tiles; ++j) {
-          for (int which = 0; which < 2; ++which) {
-            const uint32_t slot = kv_n % Cfg::kStages, ph = (kv_n / Cfg::kStages) & 1;
-            mbar_wait(&bars->kv_empty[slot], ph ^ 1);
-            mbar_arrive_expect_tx(&bars->kv_full[slot], Cfg::kTileBytes);
-            for (int pn = 0; pn < Cfg::kPanels; ++pn)
-              tma_load_3d(ring + slot * Cfg::kTileBytes + pn * Cfg::kPanelBytes,
-                          which == 0 ? &tmap_k : &tmap_v, &bars->kv_full[slot], pn * 64,
-                          it.kv_head, it.kv_row0 + j * FCP_TK);
-            ++kv_n;
-          }
+        // consumption order of the MMAs: K0, then per tile j: K_{j+1}, V_j
+        load_kv(&tmap_k, it.kv_head, it.kv_row0);
+        for (int j = 0; j < n; ++j) {
+          if (j + 1 < n) load_kv(&tmap_k, it.kv_head, it.kv_row0 + (j + 1) * FCP_TK);
+          load_kv(&tmap_v, it.kv_head, it.kv_row0 + j * FCP_TK);
         }
-        ++item_n;
+        iph ^= 1;
       }
     } else if (warp == 1 && elect_one()) {
       // ---------------------------------------------------------------- MMA issuer
-      // One elected thread.  Per KV tile j and q tile t one group: O_t += P_t(j) V_j, then
-      // S_t = Q_t K_{j+1}^T.  The barriers of the next group are probed (non-blocking) before the
-      // last kTail MMAs of the current group so the ~5-deep tcgen05 queue never drains while
-      // this thread looks at a barrier; descriptors are 32-bit adds on precomputed low words.
+      // One elected thread.  Groups of 8 MMAs in the fixed order  S_t(0) | per KV tile j:
+      // S_t(j+1) for every t, then O_t += P_t(j) V_j for every t.  The barriers of the next
+      // group are probed (non-blocking) before the last kTail MMAs of the current group so the
+      // ~5-deep tcgen05 queue never drains while this thread looks at a barrier; descriptors are
+      // 32-bit adds on precomputed low words.
       constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
       constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, 0, 1);
       constexpr int kTail = Cfg::kTail;
@@ -167,6 +177,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       auto lo_word = [](uint32_t saddr, uint32_t lbo) { return ((saddr & 0x3FFFF) >> 4) | ((lbo >> 4) << 16); };
       auto desc = [](uint32_t lo) { return ((uint64_t)kHi << 32) | lo; };
       const uint32_t q_kmaj = lo_word(smem_u32(q_smem), 16);                     // A of S (tile 0)
+      const uint32_t p_kmaj = lo_word(smem_u32(p_smem), 16);                     // A of O (tile 0)
       const uint32_t ring_kmaj = lo_word(smem_u32(ring), 16);                    // K tile, slot 0
       const uint32_t ring_mnmaj = lo_word(smem_u32(ring), Cfg::kPanelBytes);     // V tile, slot 0
 
@@ -179,10 +190,11 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
         }
       };
       auto issue_pv = [&](int t, uint32_t vslot, bool acc, int kk0, int kk1) {
-        const uint32_t b0 = ring_mnmaj + vslot * kTileStep;
+        const uint32_t a0 = p_kmaj + t * (Cfg::kPBytes >> 4), b0 = ring_mnmaj + vslot * kTileStep;
 #pragma unroll
         for (int kk = kk0; kk < kk1; ++kk)
-          umma_ts(tmem_base + (NQ + t) * 128, tmem_base + t * 128 + kk * 8,
+          umma_ss(tmem_base + (NQ + t) * 128,
+                  desc(a0 + (((kk >> 2) * Cfg::kPanelBytes + (kk & 3) * 32) >> 4)),
                   desc(b0 + kk * (2048 >> 4)), idesc_pv, (acc || kk > 0) ? 1u : 0u);
       };
       auto ring_next = [](uint32_t& s_, uint32_t& p_) {
@@ -190,10 +202,10 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       };
 
       uint32_t slot = 0, sph = 0;      // ring position / phase parity of the next tile to consume
-      uint32_t pp[NQ];                 // parity of the next p_ready phase of each q tile
+      uint32_t sfp[NQ], ppp[NQ];       // parities: S_t free (starts "already free"), P_t ready
 #pragma unroll
-      for (int t = 0; t < NQ; ++t) pp[t] = 0;
-      uint32_t iph = 0;                // item parity (q_full / o_empty / o_full)
+      for (int t = 0; t < NQ; ++t) { sfp[t] = 1; ppp[t] = 0; }
+      uint32_t iph = 0;                // item parity (q_full; o_empty of the previous item)
 #ifdef FCP_EXP_TRACE
       uint32_t tn = 0;
 #endif
@@ -201,11 +213,21 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       for (int idx = item_begin; idx < item_end; ++idx) {
         const int n = items[idx].n_kv_tiles;
         if (n == 0) continue;
+        // probes of the group that follows: S_t (tile jq) or O_t (tile jp) on ring slot (s_, p_)
+        auto test_qk = [&](int t, uint32_t s_, uint32_t p_) -> bool {
+          return mbar_test(&bars->s_free[t], sfp[t]) & (t > 0 || mbar_test(&bars->kv_full[s_], p_));
+        };
+        auto test_pv = [&](int t, uint32_t s_, uint32_t p_, int j) -> bool {
+          return mbar_test(&bars->p_ready[t], ppp[t]) & (t > 0 || mbar_test(&bars->kv_full[s_], p_)) &
+                 (j > 0 || mbar_test(&bars->o_empty[t], iph ^ 1));
+        };
         mbar_wait(&bars->q_full, iph);
         mbar_wait(&bars->kv_full[slot], sph);
-        tc_fence_after();
 #pragma unroll
         for (int t = 0; t < NQ; ++t) {
+          mbar_wait(&bars->s_free[t], sfp[t]);
+          sfp[t] ^= 1;
+          tc_fence_after();
           issue_qk(t, slot, 0, kSteps);
           umma_commit(&bars->s_full[t]);
         }
@@ -215,59 +237,59 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
         bool ok = false;               // barriers of the upcoming group already seen complete
         for (int j = 0; j < n; ++j) {
           const bool has_next = j + 1 < n;
-          const uint32_t vslot = slot, vph = sph;
-          uint32_t kslot = slot, kph = sph;
-          ring_next(kslot, kph);
+          if (has_next) {
+            // ---- S_t(j+1) = Q_t K_{j+1}^T
+#pragma unroll
+            for (int t = 0; t < NQ; ++t) {
+              if (!ok) {
+                if (t == 0) mbar_wait(&bars->kv_full[slot], sph);
+                mbar_wait(&bars->s_free[t], sfp[t]);
+              }
+              sfp[t] ^= 1;
+              tc_fence_after();
+              issue_qk(t, slot, 0, kSteps - kTail);
+              if (t + 1 < NQ) {
+                ok = test_qk(t + 1 < NQ ? t + 1 : 0, slot, sph);
+              } else {
+                uint32_t s1 = slot, p1 = sph;
+                ring_next(s1, p1);
+                ok = test_pv(0, s1, p1, j);
+              }
+              issue_qk(t, slot, kSteps - kTail, kSteps);
+              umma_commit(&bars->s_full[t]);
+            }
+            umma_commit(&bars->kv_empty[slot]);
+            if (j + 2 == n) umma_commit(&bars->q_empty);
+            ring_next(slot, sph);
+          }
+          // ---- O_t += P_t(j) V_j
 #pragma unroll
           for (int t = 0; t < NQ; ++t) {
             FTRACE(tn, 8 + 3 * t);
             if (!ok) {
-              mbar_wait(&bars->p_ready[t], pp[t]);
+              if (t == 0) mbar_wait(&bars->kv_full[slot], sph);
               if (j == 0) mbar_wait(&bars->o_empty[t], iph ^ 1);
-              if (t == 0) {
-                mbar_wait(&bars->kv_full[vslot], vph);
-                if (has_next) mbar_wait(&bars->kv_full[kslot], kph);
-              }
+              mbar_wait(&bars->p_ready[t], ppp[t]);
             }
             FTRACE(tn, 9 + 3 * t);
-            pp[t] ^= 1;
+            ppp[t] ^= 1;
             tc_fence_after();
-            // probe of the next group: (t+1, j), else (0, j+1), else none (next item: blocking)
-            auto probe_next = [&]() -> bool {
-              if (t + 1 < NQ) {
-                const int t1 = (t + 1 < NQ) ? t + 1 : 0;
-                return mbar_test(&bars->p_ready[t1], pp[t1]) &
-                       (j > 0 || mbar_test(&bars->o_empty[t1], iph ^ 1));
-              }
-              if (!has_next) return false;
-              uint32_t v1 = kslot, v1p = kph;
-              ring_next(v1, v1p);                  // V_{j+1}
-              uint32_t k2 = v1, k2p = v1p;
-              ring_next(k2, k2p);                  // K_{j+2}
-              return mbar_test(&bars->p_ready[0], pp[0]) & mbar_test(&bars->kv_full[v1], v1p) &
-                     (j + 2 >= n || mbar_test(&bars->kv_full[k2], k2p));
-            };
-            if (has_next) {
-              issue_pv(t, vslot, j > 0, 0, 8);
-              issue_qk(t, kslot, 0, kSteps - kTail);
-              ok = probe_next();
-              issue_qk(t, kslot, kSteps - kTail, kSteps);
-              umma_commit(&bars->s_full[t]);
+            issue_pv(t, slot, j > 0, 0, 8 - kTail);
+            if (t + 1 < NQ) {
+              ok = test_pv(t + 1 < NQ ? t + 1 : 0, slot, sph, j);
+            } else if (has_next) {
+              uint32_t s1 = slot, p1 = sph;
+              ring_next(s1, p1);
+              ok = (j + 2 < n) ? test_qk(0, s1, p1) : test_pv(0, s1, p1, j + 1);
             } else {
-              issue_pv(t, vslot, j > 0, 0, 8 - kTail);
-              ok = probe_next();
-              issue_pv(t, vslot, true, 8 - kTail, 8);
-              umma_commit(&bars->o_full[t]);
+              ok = false;              // next item: blocking waits
             }
+            issue_pv(t, slot, true, 8 - kTail, 8);
+            umma_commit(&bars->pv_done[t]);
             FTRACE(tn, 10 + 3 * t);
           }
-          umma_commit(&bars->kv_empty[vslot]);
+          umma_commit(&bars->kv_empty[slot]);
           ring_next(slot, sph);
-          if (has_next) {
-            umma_commit(&bars->kv_empty[kslot]);
-            ring_next(slot, sph);
-            if (j + 2 == n) umma_commit(&bars->q_empty);
-          }
 #ifdef FCP_EXP_TRACE
           ++tn;
 #endif
@@ -277,43 +299,40 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     }
   } else {
     // ------------------------------------------------------------------ softmax + epilogue
-    // kHalves warpgroups per q tile, each taking 128 / kHalves key columns of every KV tile (a
-    // warp reaches TMEM lanes 32*(warp%4)..+31 only, so each warpgroup covers all 128 query
-    // rows).  One query row per thread.  Online softmax in the log2 domain:
-    //   fast path  p = exp2(s c - m) with the running max m of the earlier tiles while the tile
-    //              max is computed on the side (no max -> exp dependency); valid as long as no
+    // One warpgroup per q tile, one query row per thread (TMEM lane = row).  Online softmax in
+    // the log2 domain, per KV tile:
+    //   fast path  p = exp2(s c - m) against the running max m of the earlier tiles while the
+    //              tile max is computed on the side (no max -> exp dependency); kept when no
     //              row of the warp exceeds m by more than 2^kRescaleThreshold;
-    //   exact path (first tile of a row, or a row that grew): tile max first, m and O rescaled.
-    constexpr int kH = Cfg::kHalves;
-    constexpr int kCW = 128 / kH;                  // key columns per thread and KV tile
-    constexpr int kOW = D / kH;                    // O columns per thread in rescale / epilogue
+    //   exact path (first tile of a row, or a row grew): tile max first, m, l and O rescaled —
+    //              S stays in registers until the path is chosen, so nothing is approximated.
+    // S is released to the MMA thread as soon as it sits in registers; P goes to shared memory
+    // after the previous O_t += P V has finished reading it.
     reg_alloc<Cfg::kRegsSoftmax>();
-    const int t = (warp - 4) / (4 * kH);           // q tile of this warp
-    const int half = ((warp - 4) >> 2) % kH;       // key-column part
+    const int t = (warp >> 2) - 1;                 // q tile of this warpgroup
     const int row = (warp & 3) * 32 + lane;        // query row = TMEM lane
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t tS = tmem_base + lane_addr + t * 128;
-    const uint32_t tP = tS + half * (kCW / 2);     // bf16 P of this thread's columns
-    const uint32_t tO = tmem_base + lane_addr + (NQ + t) * 128 + half * kOW;
-    float* xch_mine = xch + (t * 2 + half) * 128 + row;
-    const float* xch_other = xch + (t * 2 + (half ^ 1)) * 128 + row;
-    const uint32_t pair_bar = 1 + t;               // named barrier of the tile's warpgroups (kH = 2)
-    uint32_t s_ph = 0, o_ph = 0;
+    const uint32_t tO = tmem_base + lane_addr + (NQ + t) * 128;
+    const uint32_t p_row_addr = smem_u32(p_smem) + t * Cfg::kPBytes + row * 128;
+    const uint32_t swz = row & 7;
+    uint32_t s_ph = 0, pv_ph = 0;
 #ifdef FCP_EXP_TRACE
     uint32_t tn = 0;
 #endif
+    if (NQ == 2 && t == 1) named_bar_arrive(2, 256);        // tile 0 holds the MUFU token first
 
     for (int idx = item_begin; idx < item_end; ++idx) {
       const FwdItem it = items[idx];
       const int n = it.n_kv_tiles;
       const int head = it.head0 + t;
       const bool row_valid = row < it.q_rows;
-      __nv_bfloat16* o_row = o + ((int64_t)(it.q_row0 + row) * Hq + head) * D + half * kOW;
+      __nv_bfloat16* o_row = o + ((int64_t)(it.q_row0 + row) * Hq + head) * D;
       float* lse_row = lse + (int64_t)head * n_q + it.q_row0 + row;
       if (n == 0) {                                 // no visible key: o = 0, lse = -inf
         if (row_valid) {
-          for (int c = 0; c < kOW; c += 8) *reinterpret_cast<int4*>(o_row + c) = make_int4(0, 0, 0, 0);
-          if (half == 0) *lse_row = -INFINITY;
+          for (int c = 0; c < D; c += 8) *reinterpret_cast<int4*>(o_row + c) = make_int4(0, 0, 0, 0);
+          *lse_row = -INFINITY;
         }
         continue;
       }
@@ -323,145 +342,160 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       float m = -INFINITY, l = 0.f;
 
       for (int j = 0; j < n; ++j) {
-        if ((warp & (4 * kH - 1)) == 0) FTRACE(tn, 4 * t);
+        if ((warp & 3) == 0) FTRACE(tn, 4 * t);
         mbar_wait(&bars->s_full[t], s_ph);
-        if ((warp & (4 * kH - 1)) == 0) FTRACE(tn, 4 * t + 1);
+        if ((warp & 3) == 0) FTRACE(tn, 4 * t + 1);
         s_ph ^= 1;
         tc_fence_after();
-        uint32_t sr[kCW / 32][32];
+        uint32_t sr[4][32];
 #pragma unroll
-        for (int c = 0; c < kCW / 32; ++c) tmem_ld32(tS + half * kCW + c * 32, sr[c]);
+        for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, sr[c]);
         tmem_ld_wait();
-        if ((warp & (4 * kH - 1)) == 0) FTRACE(tn, 4 * t + 2);
-        const int col0 = j * FCP_TK + half * kCW;
-        if (col0 + kCW - 1 > warp_min_limit) {      // diagonal / boundary tile: mask in registers
+        tc_fence_before();
+        mbar_arrive(&bars->s_free[t]);              // S_t(j+1) may now overwrite S_t
+        if ((warp & 3) == 0) FTRACE(tn, 4 * t + 2);
+        const int col0 = j * FCP_TK;
+        if (col0 + FCP_TK - 1 > warp_min_limit) {   // diagonal / boundary tile: mask in registers
 #pragma unroll
-          for (int c = 0; c < kCW / 32; ++c)
+          for (int c = 0; c < 4; ++c)
 #pragma unroll
             for (int i = 0; i < 32; ++i)
               if (col0 + c * 32 + i > limit) sr[c][i] = 0xff800000u;   // -inf
         }
-        // ---- fast path: exponentials against the running max, tile max on the side
-        bool exact = (kH == 2) || j == 0 || __any_sync(0xffffffffu, m == -INFINITY);
-        if (!exact) {
-          float mx = -INFINITY, sum = 0.f;
+        // MUFU token: the exponentials of the two q tiles take turns (16 ex2/clk/SM bound a tile
+        // at 1024 clocks; in lockstep both warpgroups would do their loads, waits and stores at
+        // the same time and leave the MUFU idle meanwhile)
+        if (NQ == 2) named_bar_sync(2 + t, 256);
+        uint32_t pk[64];
+        float alpha = 1.f;
+        bool any_grow = false;
+        const f32x2 scale2 = pack2(scale_log2, scale_log2);
+        // p = exp2(s c - m_ref) for the whole row, packed to bf16; returns the row sum.  Packed
+        // fp32x2 FMA / ADD and the 3-input max keep the loop MUFU-bound (6 issue slots per 2
+        // elements of which 2 are MUFU).
+        bool pv_waited = j == 0;     // first tile of the item: P_t and O_t are free (epilogue waited)
+        auto exp_row = [&](float m_ref, float& mx_out, bool with_max) -> float {
+          const f32x2 negm2 = pack2(-m_ref, -m_ref);
+          f32x2 sum_a = pack2(0.f, 0.f), sum_b = sum_a;
+          float mx_a = -INFINITY, mx_b = -INFINITY;
 #pragma unroll
-          for (int c = 0; c < kCW / 32; ++c) {
+          for (int c = 0; c < 4; ++c) {
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              uint32_t pk[8];
-#pragma unroll
-              for (int i = 0; i < 8; ++i) {
-                const float s0 = __uint_as_float(sr[c][h * 16 + 2 * i]);
-                const float s1 = __uint_as_float(sr[c][h * 16 + 2 * i + 1]);
-                mx = fmaxf(mx, fmaxf(s0, s1));
-                const float p0 = fast_exp2(fmaf(s0, scale_log2, -m));
-                const float p1 = fast_exp2(fmaf(s1, scale_log2, -m));
-                sum += p0 + p1;
-                pk[i] = pack_bf16(p0, p1);
+            for (int i = 0; i < 16; i += 2) {
+              const float s0 = __uint_as_float(sr[c][2 * i]), s1 = __uint_as_float(sr[c][2 * i + 1]);
+              const float s2 = __uint_as_float(sr[c][2 * i + 2]), s3 = __uint_as_float(sr[c][2 * i + 3]);
+              if (with_max) {
+                mx_a = max3(mx_a, s0, s1);
+                mx_b = max3(mx_b, s2, s3);
               }
-              tmem_st8(tP + c * 16 + h * 8, pk);
+              float x0, x1, x2, x3;
+              unpack2(fma2(pack2(s0, s1), scale2, negm2), x0, x1);
+              unpack2(fma2(pack2(s2, s3), scale2, negm2), x2, x3);
+              const float p0 = fast_exp2(x0), p1 = fast_exp2(x1), p2 = fast_exp2(x2), p3 = fast_exp2(x3);
+              sum_a = add2(sum_a, pack2(p0, p1));
+              sum_b = add2(sum_b, pack2(p2, p3));
+              pk[c * 16 + i] = pack_bf16(p0, p1);
+              pk[c * 16 + i + 1] = pack_bf16(p2, p3);
+            }
+            // The previous O_t += P V must have finished before P_t is overwritten (it reads P
+            // from shared memory); one quarter of the exponentials later it normally has.
+            if (!pv_waited) {
+              mbar_wait(&bars->pv_done[t], pv_ph);
+              pv_ph ^= 1;
+              tc_fence_after();
+              pv_waited = true;
+            }
+            // this quarter of the P row: 4 swizzled 16-byte chunks (K-major SWIZZLE_128B operand)
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const int ch = c * 4 + q;
+              sts128(p_row_addr + (ch >> 3) * Cfg::kPanelBytes + (((ch & 7) ^ swz) << 4),
+                     pk[4 * ch], pk[4 * ch + 1], pk[4 * ch + 2], pk[4 * ch + 3]);
             }
           }
+          mx_out = fmaxf(mx_a, mx_b);
+          float lo, hi;
+          unpack2(add2(sum_a, sum_b), lo, hi);
+          return lo + hi;
+        };
+        bool exact = j == 0 || __any_sync(0xffffffffu, m == -INFINITY);
+        if (!exact) {
+          // ---- fast path: running max of the earlier tiles, tile max on the side
+          float mx;
+          const float sum = exp_row(m, mx, true);
           exact = __any_sync(0xffffffffu, mx * scale_log2 > m + kRescaleThreshold);
           if (!exact) l += sum;
         }
         if (exact) {
-          // ---- exact path: tile max first (and over both halves when kH = 2)
-          float mx = -INFINITY;
+          // ---- exact path (first tile of a row, or a row grew): tile max first
+          float mx_a = -INFINITY, mx_b = -INFINITY;
 #pragma unroll
-          for (int c = 0; c < kCW / 32; ++c)
+          for (int c = 0; c < 4; ++c)
 #pragma unroll
-            for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(sr[c][i]));
-          if (kH == 2) {
-            // The barrier also orders this part's P stores (into columns the other part loaded
-            // S from) after the other part's loads.
-            *xch_mine = mx;
-            named_bar_sync(pair_bar, 128 * kH);
-            mx = fmaxf(mx, *xch_other);
-          }
-          const float m_new = fmaxf(m, mx * scale_log2);
+            for (int i = 0; i < 32; i += 4) {
+              mx_a = max3(mx_a, __uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1]));
+              mx_b = max3(mx_b, __uint_as_float(sr[c][i + 2]), __uint_as_float(sr[c][i + 3]));
+            }
+          const float m_new = fmaxf(m, fmaxf(mx_a, mx_b) * scale_log2);
           const bool grow = m_new > m + kRescaleThreshold;   // also first finite max (m = -inf)
-          const bool any_grow = __any_sync(0xffffffffu, grow);
-          float alpha = 1.f;
+          any_grow = __any_sync(0xffffffffu, grow);
           if (grow) {
             alpha = fast_exp2(m - m_new);                   // m = -inf -> 0
             m = m_new;
           }
-          const float m_use = (m == -INFINITY) ? 0.f : m;
-          float sum = 0.f;
-#pragma unroll
-          for (int c = 0; c < kCW / 32; ++c) {
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-              uint32_t pk[8];
-#pragma unroll
-              for (int i = 0; i < 8; ++i) {
-                const float p0 = fast_exp2(fmaf(__uint_as_float(sr[c][h * 16 + 2 * i]), scale_log2, -m_use));
-                const float p1 = fast_exp2(fmaf(__uint_as_float(sr[c][h * 16 + 2 * i + 1]), scale_log2, -m_use));
-                sum += p0 + p1;
-                pk[i] = pack_bf16(p0, p1);
-              }
-              tmem_st8(tP + c * 16 + h * 8, pk);
-            }
-          }
+          float unused;
+          const float sum = exp_row((m == -INFINITY) ? 0.f : m, unused, false);
           l = l * alpha + sum;
-          if (any_grow && j > 0) {                          // rescale this thread's columns of O
-#pragma unroll
-            for (int c = 0; c < kOW / 32; ++c) {
-              uint32_t orow[32];
-              tmem_ld32(tO + c * 32, orow);
-              tmem_ld_wait();
-#pragma unroll
-              for (int i = 0; i < 32; ++i) orow[i] = __float_as_uint(__uint_as_float(orow[i]) * alpha);
-              tmem_st32(tO + c * 32, orow);
-            }
-          }
         }
-        tmem_st_wait();
+        if (NQ == 2) named_bar_arrive(2 + (t ^ 1), 256);   // pass the MUFU token
+        if (any_grow && j > 0) {                            // rescale the running O row
+#pragma unroll
+          for (int c = 0; c < D / 32; ++c) {
+            uint32_t orow[32];
+            tmem_ld32(tO + c * 32, orow);
+            tmem_ld_wait();
+#pragma unroll
+            for (int i = 0; i < 32; ++i) orow[i] = __float_as_uint(__uint_as_float(orow[i]) * alpha);
+            tmem_st32(tO + c * 32, orow);
+          }
+          tmem_st_wait();
+        }
+        fence_proxy_async_smem();
         tc_fence_before();
         mbar_arrive(&bars->p_ready[t]);
-        if ((warp & (4 * kH - 1)) == 0) FTRACE(tn, 4 * t + 3);
-        if (warp == 5) FTRACE(tn, 14);
-        if (warp == 7) FTRACE(tn, 15);
+        if ((warp & 3) == 0) FTRACE(tn, 4 * t + 3);
 #ifdef FCP_EXP_TRACE
         ++tn;
 #endif
       }
 
       // epilogue: o = O / l, lse = ln2 * (m + log2 l)
-      if (kH == 2) {
-        *xch_mine = l;
-        named_bar_sync(pair_bar, 128 * kH);
-        l += *xch_other;
-      }
-      mbar_wait(&bars->o_full[t], o_ph);
-      o_ph ^= 1;
+      mbar_wait(&bars->pv_done[t], pv_ph);
+      pv_ph ^= 1;
       tc_fence_after();
       const float inv = l > 0.f ? 1.f / l : 0.f;
 #pragma unroll
-      for (int c = 0; c < kOW / 32; ++c) {
+      for (int c = 0; c < D / 32; ++c) {
         uint32_t orow[32];
         tmem_ld32(tO + c * 32, orow);
         tmem_ld_wait();
         if (row_valid) {
 #pragma unroll
           for (int i = 0; i < 4; ++i) {
-            int4 pk;
-            pk.x = pack_bf16(__uint_as_float(orow[8 * i + 0]) * inv, __uint_as_float(orow[8 * i + 1]) * inv);
-            pk.y = pack_bf16(__uint_as_float(orow[8 * i + 2]) * inv, __uint_as_float(orow[8 * i + 3]) * inv);
-            pk.z = pack_bf16(__uint_as_float(orow[8 * i + 4]) * inv, __uint_as_float(orow[8 * i + 5]) * inv);
-            pk.w = pack_bf16(__uint_as_float(orow[8 * i + 6]) * inv, __uint_as_float(orow[8 * i + 7]) * inv);
-            *reinterpret_cast<int4*>(o_row + c * 32 + i * 8) = pk;
+            int4 v;
+            v.x = pack_bf16(__uint_as_float(orow[8 * i + 0]) * inv, __uint_as_float(orow[8 * i + 1]) * inv);
+            v.y = pack_bf16(__uint_as_float(orow[8 * i + 2]) * inv, __uint_as_float(orow[8 * i + 3]) * inv);
+            v.z = pack_bf16(__uint_as_float(orow[8 * i + 4]) * inv, __uint_as_float(orow[8 * i + 5]) * inv);
+            v.w = pack_bf16(__uint_as_float(orow[8 * i + 6]) * inv, __uint_as_float(orow[8 * i + 7]) * inv);
+            *reinterpret_cast<int4*>(o_row + c * 32 + i * 8) = v;
           }
         }
       }
       tc_fence_before();
       mbar_arrive(&bars->o_empty[t]);
-      if (row_valid && half == 0) *lse_row = l > 0.f ? kLn2 * (m + __log2f(l)) : -INFINITY;
-      // the exchange slot is rewritten at the next item's first tile: keep the parts together
-      if (kH == 2) named_bar_sync(pair_bar, 128 * kH);
+      if (row_valid) *lse_row = l > 0.f ? kLn2 * (m + __log2f(l)) : -INFINITY;
     }
+    if (NQ == 2 && t == 0) named_bar_sync(2, 256);          // consume tile 1's last token
   }
 
   tc_fence_before();

@@ -171,8 +171,8 @@ class Plan:
         self.doc_lengths = d.copy()
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            _lib().fcp_plan_destroy(self._h)
+        if getattr(self, "_h", None) and _LIB is not None:   # module globals vanish at shutdown
+            _LIB.fcp_plan_destroy(self._h)
             self._h = None
 
     def shards(self, rank=-1):
@@ -259,8 +259,8 @@ class Sched:
         return cls(h, n_q_heads, n_kv_heads, head_dim)
 
     def __del__(self):
-        if getattr(self, "_h", None):
-            _lib().fcp_sched_destroy(self._h)
+        if getattr(self, "_h", None) and _LIB is not None:
+            _LIB.fcp_sched_destroy(self._h)
             self._h = None
 
     def info(self):

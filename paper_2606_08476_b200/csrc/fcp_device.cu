@@ -7,19 +7,22 @@
 #include <cstring>
 
 #include "fcp_internal.h"
+#include "fcp_sm100.cuh"
 
 namespace {
 
 // ------------------------------------------------------------------------------------------
 // KV gather: a handful of contiguous row ranges of K and V are copied into k_out / v_out.
-// Everything is expressed in 16-byte chunks.  A CTA copies "slabs" of kSlab chunks; all loads
-// of a thread are issued before its stores (8 x 16 B in flight per thread), loads bypass L1,
-// stores are streaming.  HBM-bound: 2 tensors x (read + write) x rows x Hkv*D*2 bytes.
+// Everything is expressed in 16-byte chunks; the destination is cut in 32 KB slabs that the
+// CTAs take round-robin.  One thread per CTA drives the copy engine: cp.async.bulk global ->
+// shared (mbarrier complete_tx) through a 3-slot ring, then cp.async.bulk shared -> global, so
+// that 64 KB of loads per CTA (two CTAs per SM) are in flight with no register staging.
+// HBM-bound: 2 tensors x (read + write) x rows x Hkv*D*2 bytes.
 // ------------------------------------------------------------------------------------------
 constexpr int kMaxRanges = 120;
-constexpr int kGatherThreads = 256;
-constexpr int kGatherUnroll = 8;
-constexpr int kSlab = kGatherThreads * kGatherUnroll;   // 2048 chunks = 32 KB
+constexpr int kSlab = 2048;                 // chunks per slab = 32 KB
+constexpr int kGatherStages = 3;
+constexpr int kGatherSmem = kGatherStages * kSlab * 16 + 64;
 
 struct GatherRanges {
   int32_t n;
@@ -28,52 +31,66 @@ struct GatherRanges {
   int64_t src0[kMaxRanges];       // first source chunk of each range
 };
 
-__device__ __forceinline__ int4 ld_stream(const int4* p) {
-  int4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.L2::128B.v4.s32 {%0,%1,%2,%3}, [%4];"
-               : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
-               : "l"(p));
-  return r;
-}
-__device__ __forceinline__ void st_stream(int4* p, const int4& v) {
-  asm volatile("st.global.cs.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y),
-               "r"(v.z), "r"(v.w)
-               : "memory");
-}
-
-__global__ void __launch_bounds__(kGatherThreads)
+__global__ void __launch_bounds__(32)
 fcp_kv_gather_kernel(const int4* __restrict__ K, const int4* __restrict__ V,
                      int4* __restrict__ k_out, int4* __restrict__ v_out,
                      const __grid_constant__ GatherRanges rg) {
+  extern __shared__ __align__(128) uint8_t gsm[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(gsm + kGatherStages * kSlab * 16);
+  if (threadIdx.x != 0) return;
+  using namespace fcp;
+  for (int i = 0; i < kGatherStages; ++i) mbar_init(&full[i], 1);
+  fence_barrier_init();
   const int64_t total = rg.dst0[rg.n];
   const int64_t n_slabs = (total + kSlab - 1) / kSlab;
-  for (int64_t slab = blockIdx.x; slab < 2 * n_slabs; slab += gridDim.x) {
+  const int64_t n_work = 2 * n_slabs;                       // K slabs then V slabs
+  const int64_t n_mine = blockIdx.x < n_work ? (n_work - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+
+  // issue the loads of my w-th slab into ring slot w % kGatherStages
+  auto load = [&](int64_t w) {
+    const int64_t slab = blockIdx.x + w * gridDim.x;
     const bool is_v = slab >= n_slabs;
     const int64_t c0 = (is_v ? slab - n_slabs : slab) * kSlab;
+    const int64_t c1 = c0 + kSlab < total ? c0 + kSlab : total;
     const int4* __restrict__ src = is_v ? V : K;
-    int4* __restrict__ dst = is_v ? v_out : k_out;
-    // range that holds the slab's first chunk (uniform over the CTA)
-    int lo = 0, hi = rg.n - 1;
+    const int st = (int)(w % kGatherStages);
+    uint8_t* dst = gsm + st * kSlab * 16;
+    mbar_arrive_expect_tx(&full[st], (uint32_t)(c1 - c0) * 16);
+    int lo = 0, hi = rg.n - 1;                              // range that holds chunk c0
     while (lo < hi) {
       const int mid = (lo + hi + 1) >> 1;
       if (rg.dst0[mid] <= c0) lo = mid; else hi = mid - 1;
     }
-    int4 val[kGatherUnroll];
-    int r = lo;
-#pragma unroll
-    for (int u = 0; u < kGatherUnroll; ++u) {
-      const int64_t c = c0 + u * kGatherThreads + threadIdx.x;
-      if (c < total) {
-        while (c >= rg.dst0[r + 1]) ++r;
-        val[u] = ld_stream(src + rg.src0[r] + (c - rg.dst0[r]));
+    for (int64_t c = c0; c < c1; ++lo) {                    // a slab may straddle range borders
+      const int64_t e = rg.dst0[lo + 1] < c1 ? rg.dst0[lo + 1] : c1;
+      if (e > c) {
+        bulk_load_1d(dst + (c - c0) * 16, src + rg.src0[lo] + (c - rg.dst0[lo]), (uint32_t)(e - c) * 16,
+                     &full[st]);
+        c = e;
       }
     }
-#pragma unroll
-    for (int u = 0; u < kGatherUnroll; ++u) {
-      const int64_t c = c0 + u * kGatherThreads + threadIdx.x;
-      if (c < total) st_stream(dst + c, val[u]);
+  };
+  const int64_t ahead = kGatherStages - 1;
+  for (int64_t w = 0; w < ahead && w < n_mine; ++w) load(w);
+  for (int64_t w = 0; w < n_mine; ++w) {
+    const int64_t slab = blockIdx.x + w * gridDim.x;
+    const bool is_v = slab >= n_slabs;
+    const int64_t c0 = (is_v ? slab - n_slabs : slab) * kSlab;
+    const int64_t c1 = c0 + kSlab < total ? c0 + kSlab : total;
+    const int st = (int)(w % kGatherStages);
+    if (w + ahead < n_mine) {
+      // slot (w + ahead) % stages was read by the store of slab w - 1: wait for that read
+      asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+      load(w + ahead);
     }
+    mbar_wait(&full[st], (uint32_t)((w / kGatherStages) & 1));
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(
+                     (is_v ? v_out : k_out) + c0),
+                 "r"(smem_u32(gsm + st * kSlab * 16)), "r"((uint32_t)(c1 - c0) * 16)
+                 : "memory");
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
   }
+  asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // ------------------------------------------------------------------------------------------
@@ -200,8 +217,15 @@ extern "C" int fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, 
     rg.dst0[rg.n] = c;
     const int64_t slabs = 2 * ((c + kSlab - 1) / kSlab);
     if (slabs == 0) continue;
-    const int grid = (int)std::min<int64_t>(slabs, (int64_t)num_sms * 8);
-    fcp_kv_gather_kernel<<<grid, kGatherThreads, 0, (cudaStream_t)stream>>>(
+    static bool attr_set = false;
+    if (!attr_set) {
+      if (cudaFuncSetAttribute(fcp_kv_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                               kGatherSmem) != cudaSuccess)
+        return FCP_CUDA;
+      attr_set = true;
+    }
+    const int grid = (int)std::min<int64_t>(slabs, (int64_t)num_sms * 2);
+    fcp_kv_gather_kernel<<<grid, 32, kGatherSmem, (cudaStream_t)stream>>>(
         reinterpret_cast<const int4*>(K), reinterpret_cast<const int4*>(V),
         reinterpret_cast<int4*>(k_out) + dst_row * cpr, reinterpret_cast<int4*>(v_out) + dst_row * cpr,
         rg);

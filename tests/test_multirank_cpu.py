@@ -1,0 +1,76 @@
+"""N > 1 path of bench.py on CPU: two gloo ranks (no GPU).  The hot path shards over GPUs as
+independent packed batches (weak scaling, no data-path collective — DESIGN.md section 6); what
+crosses ranks is only the timing / flop aggregation, which is what these tests exercise, plus
+the host planner running in both processes on their own batch."""
+import os
+import socket
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, out):
+    import torch.distributed as dist
+    import bench
+    import fcp_inputs
+    import paper_2606_08476_b200 as fcp
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        # every rank plans its own packed batch (seed + rank), as run_fcp does
+        cfg = fcp_inputs.CONFIGS["8b"]
+        d = fcp_inputs.doc_lengths("8b", bench.rank_seed(0, rank))
+        plan = fcp.Plan(d, cfg.N)
+        st = plan.stats()
+        assert st["context_len"] == cfg.C and st["tokens_per_rank"] == cfg.C // cfg.N
+        f_fwd, f_bwd = bench.useful_flops(cfg, d)
+        my_flops = float(f_fwd + f_bwd)
+        my_ms = 10.0 * (rank + 1)                    # rank 1 is the slow one
+        value, ms = bench.job_throughput(my_flops, my_ms, dist, "cpu")
+        total = bench.over_ranks(my_flops, "sum", dist, "cpu")
+        n_docs_max = bench.over_ranks(float(len(d)), "max", dist, "cpu")
+        out.put((rank, value, ms, total, my_flops, len(d), n_docs_max))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_two_gloo_ranks_aggregate_whole_job_throughput():
+    import torch.multiprocessing as mp
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(out.get(timeout=180) for _ in procs)
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    (_, v0, ms0, tot0, f0, n0, nm0), (_, v1, ms1, tot1, f1, n1, nm1) = res
+    # time = max over ranks, work = sum over ranks, identical on both ranks
+    assert ms0 == ms1 == 20.0
+    assert tot0 == tot1 == pytest.approx(f0 + f1)
+    assert v0 == v1 == pytest.approx((f0 + f1) / 20e-3 / 1e12)
+    # the two ranks really worked on different batches
+    assert (f0, n0) != (f1, n1)
+    assert nm0 == nm1 == max(n0, n1)
+
+
+def test_single_process_is_identity():
+    import bench
+    assert bench.over_ranks(3.5, "max") == 3.5
+    v, ms = bench.job_throughput(2e12, 1000.0)
+    assert ms == 1000.0 and v == pytest.approx(2.0)

@@ -375,11 +375,15 @@ def run_fcp(args):
     if rank == 0:
         st = w.stats
         kv_b = 2 * row_bytes                                  # K and V, one pass, per token
+        # dram__bytes_read + dram__bytes_write of the dominant kernel from the committed ncu capture
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "bwd_main_dram_bytes.json")
+        tp = os.path.join(ROOT, "profiles", "r1c_traffic.csv")
         if os.path.exists(tp):
             try:
-                traffic = json.load(open(tp)).get(args.config)
+                import csv
+                for row in csv.DictReader(open(tp)):
+                    if row["config"] == args.config and row["kernel"] == "fcp_attn_bwd_main":
+                        traffic = int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
             except Exception:
                 traffic = None
         line = {

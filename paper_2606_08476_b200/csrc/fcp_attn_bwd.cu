@@ -9,8 +9,9 @@
 //                        tile of one KV segment for one kv head; it loops over every (shard,
 //                        64-row q tile, query head of the GQA group) that sees the tile and keeps
 //                        dK, dV in TMEM for the whole item (the GQA sum costs nothing, no atomics):
-//        warp 0      TMA producer  K,V tile once per item; Q, dO, (lse,delta) per iteration (3 stages)
-//        warp 1      MMA issuer    S^T = K Q^T, dP^T = V dO^T (SS);  dV += P^T dO, dK += dS^T Q
+//      (roles; the control warpgroup is mapped to the highest warp ids, see the kernel)
+//        role 0      TMA producer  K,V tile once per item; Q, dO, (lse,delta) per iteration (3 stages)
+//        role 1      MMA issuer    S^T = K Q^T, dP^T = V dO^T (SS);  dV += P^T dO, dK += dS^T Q
 //                                  (A from TMEM);  dQ^T = K^T dS^T (SS, dS^T staged in smem)
 //        warps 4-11  softmax       two warpgroups, 32 q columns each, one KV row per thread:
 //                                  P^T = exp2(S^T c - lse), mask, dS^T = P^T o (dP^T - delta);
@@ -267,6 +268,10 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
 
   const int warp = threadIdx.x >> 5;
   const int lane = threadIdx.x & 31;
+  // Role of the warp.  The control warpgroup sits in the HIGHEST warp ids (12-15): the warp
+  // scheduler favours high ids, and the single MMA-issuing thread must never queue behind the
+  // softmax warps of its sub-partition.  TMEM lane quarters depend on warp % 4 only.
+  const int role = (warp + 4) & 15;   // 0 producer, 1 MMA, 4-11 softmax, 12-15 dQ drain
 
   if (threadIdx.x == 0) {
     mbar_init(&bars->kv_full, 1);
@@ -285,16 +290,16 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     mbar_init(&bars->dkv_free, 256);
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc<512>(&bars->tmem_base);
+  if (role == 1) tmem_alloc<512>(&bars->tmem_base);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = bars->tmem_base;
   const int item_begin = cta_off[blockIdx.x], item_end = cta_off[blockIdx.x + 1];   // this CTA's work list
 
-  if (warp < 4) {
+  if (role < 4) {
     reg_dealloc<Cfg::kRegsCtl>();
-    if (warp == 0 && lane == 0) {
+    if (role == 0 && lane == 0) {
       // ---------------------------------------------------------------- TMA producer
       prefetch_tmap(&tmap_q);
       prefetch_tmap(&tmap_do);
@@ -329,7 +334,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         }
         ++m;
       }
-    } else if (warp == 1 && elect_one()) {
+    } else if (role == 1 && elect_one()) {
       // ---------------------------------------------------------------- MMA issuer
       // One elected thread (elect.sync compiles to straight-line UTCHMMA).  The tcgen05 queue is
       // only about 5 MMAs deep, so issue runs at the pace of execution; the barriers of the next
@@ -355,6 +360,9 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       constexpr uint32_t kStageStep = Cfg::kStage >> 4, kDoStep = Cfg::kQTile >> 4;
       // ring state of iteration n: stage index, parity of the stage's phase, n & 1
       uint32_t st = 0, sph = 0, b = 0, mph = 0;
+#ifdef FCP_EXP_TRACE
+      uint32_t tn_ = 0;
+#endif
 
       // S^T = K Q^T  or  dP^T = V dO^T : A = kv tile (K-major), B = q/dO tile (K-major)
       auto issue_kq = [&](uint32_t d_col, uint32_t a_lo, uint32_t b_lo, int kk0, int kk1) {
@@ -391,6 +399,8 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
               mbar_wait(&bars->dpt_free, b);     // softmax(n) holds dP^T(n) in registers
             }
             tc_fence_after();
+            TRACE(tn_, 1);
+            TRACEV(tn_, 12, ok_a);
             const uint32_t q_lo = q_kmaj0 + st1 * kStageStep;
             issue_kq(Cfg::kColS + (b ^ 1) * 64, k_kmaj, q_lo, 0, kSteps);
             issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, 0, kSteps - kTail);
@@ -398,6 +408,8 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
                    (i > 0 || mbar_test(&bars->dkv_free, mph ^ 1));
             issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, kSteps - kTail, kSteps);
             umma_commit(&bars->st_full);
+            TRACE(tn_, 2);
+            TRACEV(tn_, 13, ok_b);
           }
           if (!ok_b) {
             mbar_wait(&bars->p_ready, b);
@@ -405,6 +417,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
             mbar_wait(&bars->dq_free, b ^ 1);
           }
           tc_fence_after();
+          TRACE(tn_, 3);
           // P^T / dS^T of q columns [32h, 32h+32) live in columns [32h, 32h+16) / [32h+16, 32h+32)
           // of the S^T buffer: each softmax warpgroup overwrites only the columns it has loaded
           const uint32_t tP = tmem_base + Cfg::kColS + b * 64, tDS = tP + 16;
@@ -434,6 +447,10 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
           umma_commit(&bars->qdo_free[st]);
           umma_commit(&bars->ds_free[b]);
           umma_commit(&bars->dq_full);
+          TRACE(tn_, 4);
+#ifdef FCP_EXP_TRACE
+          ++tn_;
+#endif
           st = st1;
           sph = sph1;
           b ^= 1;
@@ -443,13 +460,13 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         mph ^= 1;
       }
     }
-  } else if (warp < 12) {
+  } else if (role < 12) {
     // ------------------------------------------------------------------ softmax / dS
     // Two warpgroups: warps 4-7 take q columns 0..31 of the 64-column tile, warps 8-11 take
     // columns 32..63 (a warp reaches TMEM lanes 32*(warp%4)..+31 only, so each warpgroup covers
     // all 128 KV rows).
     reg_alloc<Cfg::kRegsSoftmax>();
-    const int half = (warp - 4) >> 2;                  // 0 or 1
+    const int half = (role - 4) >> 2;                  // 0 or 1
     const int row = (warp & 3) * 32 + lane;            // KV row of the tile = TMEM lane
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t stat_base = smem_u32(stat_smem) + half * 32 * 8;
@@ -476,9 +493,9 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         const int q_pos = w.q_pos() + half * 32;       // position of this half's first column
         // mask needed when some (kv, q) pair of this warp's rows is invisible
         const bool need_mask = (warp_kv_max > q_pos) || (it.kv_rows < 128);
-        if (warp == 4) TRACE(n, 5);
+        if (role == 4) TRACE(n, 5);
         mbar_wait(&bars->st_full, n & 1);
-        if (warp == 4) TRACE(n, 6);
+        if (role == 4) TRACE(n, 6);
         tc_fence_after();
         uint32_t s[32], dp[32];
         tmem_ld32(tS + half * 32, s);
@@ -488,7 +505,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         tmem_ld_wait();
         tc_fence_before();
         mbar_arrive(&bars->dpt_free);                              // dP^T (and S^T) now in registers
-        if (warp == 4) TRACE(n, 7);
+        if (role == 4) TRACE(n, 7);
         const uint32_t stat_addr = stat_base + st * Cfg::kStat;
         const uint32_t ds_row_addr = ds_base + (n & 1) * Cfg::kDS;
         if (need_mask)
@@ -501,7 +518,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         tmem_st_wait();
         tc_fence_before();
         mbar_arrive(&bars->p_ready);
-        if (warp == 4) TRACE(n, 8);
+        if (role == 4) TRACE(n, 8);
       }
       // item epilogue: dV (half 0) / dK (half 1) rows out of TMEM
       mbar_wait(&bars->dkv_full, m & 1);
@@ -544,15 +561,15 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     const int drow = (warp & 3) * 32 + lane;           // d index = TMEM lane of dQ^T
     const uint32_t tDQ = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + Cfg::kColDQ;
     const uint32_t dq_addr = smem_u32(dq_smem) + drow * 4;
-    const bool leader = threadIdx.x == 12 * 32;
+    const bool leader = role == 12 && lane == 0;
     uint32_t n = 0;
     for (int idx = item_begin; idx < item_end; ++idx) {
       const BwdItem it = items[idx];
       if (it.n_iters == 0) continue;
       for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
-        if (warp == 12) TRACE(n, 9);
+        if (role == 12) TRACE(n, 9);
         mbar_wait(&bars->dq_full, n & 1);
-        if (warp == 12) TRACE(n, 10);
+        if (role == 12) TRACE(n, 10);
         tc_fence_after();
         uint32_t acc[2][32];
         tmem_ld32(tDQ, acc[0]);
@@ -560,7 +577,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         tmem_ld_wait();
         tc_fence_before();
         mbar_arrive(&bars->dq_free);
-        if (warp == 12) TRACE(n, 11);
+        if (role == 12) TRACE(n, 11);
         if (leader) bulk_wait_read0();                  // previous reduce has read the staging
         named_bar_sync(1, 128);
         if (drow < D) {
@@ -582,7 +599,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) {
+  if (role == 1) {
     __syncwarp();
     tmem_dealloc<512>(tmem_base);
   }

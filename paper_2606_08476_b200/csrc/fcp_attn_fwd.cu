@@ -47,6 +47,10 @@ using namespace fcp;
 
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
+#ifndef FCP_TOKEN_QUARTER
+#define FCP_TOKEN_QUARTER 0
+#endif
+constexpr int kTokenQuarter = FCP_TOKEN_QUARTER;   // quarter of the exponential loop after which the MUFU token moves on
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: rescale O only when the max grew by > 2^8
 
 template <int D, int NQ>
@@ -366,6 +370,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // at 1024 clocks; in lockstep both warpgroups would do their loads, waits and stores at
         // the same time and leave the MUFU idle meanwhile)
         if (NQ == 2) named_bar_sync(2 + t, 256);
+        if (NQ == 2 && kTokenQuarter < 0) named_bar_arrive(2 + (t ^ 1), 256);
         uint32_t pk[64];
         float alpha = 1.f;
         bool any_grow = false;
@@ -374,6 +379,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // fp32x2 FMA / ADD and the 3-input max keep the loop MUFU-bound (6 issue slots per 2
         // elements of which 2 are MUFU).
         bool pv_waited = j == 0;     // first tile of the item: P_t and O_t are free (epilogue waited)
+        bool token_passed = NQ != 2 || kTokenQuarter < 0;
         auto exp_row = [&](float m_ref, float& mx_out, bool with_max) -> float {
           const f32x2 negm2 = pack2(-m_ref, -m_ref);
           f32x2 sum_a = pack2(0.f, 0.f), sum_b = sum_a;
@@ -412,6 +418,13 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
               sts128(p_row_addr + (ch >> 3) * Cfg::kPanelBytes + (((ch & 7) ^ swz) << 4),
                      pk[4 * ch], pk[4 * ch + 1], pk[4 * ch + 2], pk[4 * ch + 3]);
             }
+            // hand the MUFU token on part-way: the other tile starts its exponentials while
+            // this one finishes (two warps per sub-partition keep the MUFU saturated; one alone
+            // is latency-bound)
+            if (c == kTokenQuarter && !token_passed) {
+              named_bar_arrive(2 + (t ^ 1), 256);
+              token_passed = true;
+            }
           }
           mx_out = fmaxf(mx_a, mx_b);
           float lo, hi;
@@ -447,7 +460,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
           const float sum = exp_row((m == -INFINITY) ? 0.f : m, unused, false);
           l = l * alpha + sum;
         }
-        if (NQ == 2) named_bar_arrive(2 + (t ^ 1), 256);   // pass the MUFU token
         if (any_grow && j > 0) {                            // rescale the running O row
 #pragma unroll
           for (int c = 0; c < D / 32; ++c) {

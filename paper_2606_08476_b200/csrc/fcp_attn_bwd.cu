@@ -2,7 +2,7 @@
 // for sm_100a.
 //
 // Three launches:
-//   1. fcp_bwd_prep      delta = rowsum(dO o O); (lse*log2e, delta) into a 64-row-padded scratch
+//   1. fcp_bwd_prep      zeroes the fp32 dq accumulator; delta = rowsum(dO o O); (lse*log2e, delta) into a 64-row-padded scratch
 //                        so that every q tile's statistics are one aligned 512-byte bulk copy;
 //                        padding rows get lse = +inf (P = 0: they contribute nothing).
 //   2. fcp_attn_bwd_main one persistent CTA per SM, 16 warps.  A work item is one 128-row KV
@@ -62,8 +62,14 @@ template <int D>
 __global__ void __launch_bounds__(256)
 fcp_bwd_prep(const __nv_bfloat16* __restrict__ o, const __nv_bfloat16* __restrict__ dO,
              const float* __restrict__ lse, const int32_t* __restrict__ tile_meta,
-             float2* __restrict__ lsed, int64_t n_q, int64_t n_q_pad, int Hq) {
+             float2* __restrict__ lsed, float4* __restrict__ dq_acc, int64_t n_q, int64_t n_q_pad,
+             int Hq) {
   const int tile = blockIdx.x, head = blockIdx.y;
+  // zero this (q tile, head) block of the fp32 dQ accumulator: saves a separate memset pass
+  {
+    float4* z = dq_acc + ((int64_t)head * n_q_pad + (int64_t)tile * FCP_BQ) * (D / 4);
+    for (int i = threadIdx.x; i < FCP_BQ * D / 4; i += blockDim.x) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+  }
   const int row0 = tile_meta[2 * tile], valid = tile_meta[2 * tile + 1];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   constexpr int kPerLane = D / 32;                       // 2 or 4 bf16 per lane
@@ -615,13 +621,11 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
   float2* lsed = reinterpret_cast<float2*>(ws + s->off_lsed);
   float* dq_acc = reinterpret_cast<float*>(ws + s->off_dq);
   const int n_pad_tiles = (int)(s->n_q_pad / FCP_BQ);
-  const size_t dq_bytes = (size_t)s->Hq * s->n_q_pad * D * sizeof(float);
 
   if (n_pad_tiles > 0) {
-    if (cudaMemsetAsync(dq_acc, 0, dq_bytes, st) != cudaSuccess) return FCP_CUDA;
     fcp_bwd_prep<D><<<dim3(n_pad_tiles, s->Hq), 256, 0, st>>>(
         static_cast<const __nv_bfloat16*>(a->o), static_cast<const __nv_bfloat16*>(dO), a->lse,
-        tile_meta, lsed, s->n_q, s->n_q_pad, s->Hq);
+        tile_meta, lsed, reinterpret_cast<float4*>(dq_acc), s->n_q, s->n_q_pad, s->Hq);
     if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
   }
   const int n_items = (int)s->bwd.size();

@@ -370,6 +370,13 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       uint32_t tn_ = 0;
 #endif
 
+      // Keeps ptxas from hoisting the eight 64-bit A descriptors of a product out of the loop
+      // into general registers (16 R2UR per product and iteration); from an opaque base they
+      // are one R2UR plus uniform adds, like the B descriptors.
+      auto opaque = [](uint32_t x) {
+        asm volatile("" : "+r"(x));
+        return x;
+      };
       // S^T = K Q^T  or  dP^T = V dO^T : A = kv tile (K-major), B = q/dO tile (K-major)
       auto issue_kq = [&](uint32_t d_col, uint32_t a_lo, uint32_t b_lo, int kk0, int kk1) {
 #pragma unroll
@@ -408,11 +415,12 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
             TRACE(tn_, 1);
             TRACEV(tn_, 12, ok_a);
             const uint32_t q_lo = q_kmaj0 + st1 * kStageStep;
-            issue_kq(Cfg::kColS + (b ^ 1) * 64, k_kmaj, q_lo, 0, kSteps);
-            issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, 0, kSteps - kTail);
+            const uint32_t v_lo = opaque(v_kmaj);
+            issue_kq(Cfg::kColS + (b ^ 1) * 64, opaque(k_kmaj), q_lo, 0, kSteps);
+            issue_kq(Cfg::kColDP, v_lo, q_lo + kDoStep, 0, kSteps - kTail);
             ok_b = mbar_test(&bars->p_ready, b) & mbar_test(&bars->dq_free, b ^ 1) &
                    (i > 0 || mbar_test(&bars->dkv_free, mph ^ 1));
-            issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, kSteps - kTail, kSteps);
+            issue_kq(Cfg::kColDP, v_lo, q_lo + kDoStep, kSteps - kTail, kSteps);
             umma_commit(&bars->st_full);
             TRACE(tn_, 2);
             TRACEV(tn_, 13, ok_b);
@@ -439,16 +447,17 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
                     desc(q_lo + kk * (2048 >> 4)), idesc_kv, (i > 0 || kk > 0) ? 1u : 0u);
           // dQ^T = K^T dS^T : A = K tile as MN-major [K=kv][M=d], B = dS^T smem MN-major [K=kv][N=q]
           const uint32_t ds_lo = ds_mnmaj + b * (Cfg::kDS >> 4);
+          const uint32_t kt_lo = opaque(k_mnmaj);
 #pragma unroll
           for (int kk = 0; kk < 8 - kTail; ++kk)
-            umma_ss(tmem_base + Cfg::kColDQ, desc(k_mnmaj + kk * (2048 >> 4)),
+            umma_ss(tmem_base + Cfg::kColDQ, desc(kt_lo + kk * (2048 >> 4)),
                     desc(ds_lo + kk * (2048 >> 4)), idesc_dq, kk > 0);
           ok_a = false;
           if (i + 2 < I)
             ok_a = mbar_test(&bars->qdo_full[st2], sph2) & mbar_test(&bars->dpt_free, b ^ 1);
 #pragma unroll
           for (int kk = 8 - kTail; kk < 8; ++kk)
-            umma_ss(tmem_base + Cfg::kColDQ, desc(k_mnmaj + kk * (2048 >> 4)),
+            umma_ss(tmem_base + Cfg::kColDQ, desc(kt_lo + kk * (2048 >> 4)),
                     desc(ds_lo + kk * (2048 >> 4)), idesc_dq, 1u);
           umma_commit(&bars->qdo_free[st]);
           umma_commit(&bars->ds_free[b]);

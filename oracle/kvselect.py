@@ -125,3 +125,16 @@ def rank_layout(p: Plan, rank: int) -> RankLayout:
     i32 = lambda a: np.asarray(a, dtype=np.int32)
     return RankLayout(i32(cu_q), i32(ppos), i32(sseg), i32(cu_k), i32(kv_src), i32(kv_len),
                       i32(seg_doc))
+
+
+def scatter_add(p: Plan, rank: int, dkv_rank: np.ndarray, dKV_global: np.ndarray) -> None:
+    """dKV reduction of one rank (the gradients of the communicated KV are
+    reduce-scattered back to the ranks that own the tokens; the inverse of the KV selection of
+    PAPER.md:111-113).  `dkv_rank` [n_kv_r, Hkv, D] holds the rank's own contribution in
+    gathered-KV order; row i is added to row gather_index(p, rank)[i] of `dKV_global`
+    [C, Hkv, D], in place.  Plain definition: global dK = sum over ranks of this scatter-add."""
+    gi = gather_index(p, rank)
+    if dkv_rank.shape[0] != gi.shape[0]:
+        raise ValueError("dkv_rank has %d rows, the rank gathers %d" % (dkv_rank.shape[0], gi.shape[0]))
+    # the gathered rows of one rank are distinct tokens, so a plain indexed add is exact
+    dKV_global[gi] += dkv_rank

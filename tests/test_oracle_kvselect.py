@@ -1,5 +1,6 @@
 """Pins for oracle/kvselect.py: pair-by-pair brute force of the needed-key
 set, Eq.5 <= Eq.4, the whole-document and N=1 special cases."""
+import pytest
 import numpy as np
 
 from oracle import planner as P
@@ -78,3 +79,58 @@ def test_rank_layout_tiny():
         lay = KV.rank_layout(pl, r)
         idx = np.concatenate([np.arange(s, s + l) for s, l in zip(lay.kv_src_start, lay.kv_len)])
         assert (idx == KV.gather_index(pl, r)).all()
+
+
+def test_scatter_add_is_the_inverse_of_the_gather_brute_force():
+    """kvselect.scatter_add pinned by a token-by-token loop: every gathered row lands on the
+    global token it was gathered from, rows of different ranks that hit the same token add up,
+    tokens no rank gathered stay untouched."""
+    rng = np.random.default_rng(3)
+    d = [37, 5, 20, 2]
+    for N, strategy in ((2, 0), (4, 1), (1, 2)):
+        pl = P.plan(d, N, strategy=strategy)
+        C = sum(d)
+        want = np.zeros((C, 2, 3))
+        got = np.zeros((C, 2, 3))
+        touched = np.zeros(C, dtype=int)
+        for r in range(N):
+            gi = KV.gather_index(pl, r)
+            part = rng.standard_normal((len(gi), 2, 3))
+            KV.scatter_add(pl, r, part, got)
+            for row, tok in enumerate(gi):          # brute force
+                want[tok] += part[row]
+                touched[tok] += 1
+        assert np.array_equal(got, want)
+        # every token is gathered by its owner at least (a token sees itself)
+        assert (touched >= 1).all()
+    with pytest.raises(ValueError):
+        KV.scatter_add(pl, 0, np.zeros((1, 2, 3)), np.zeros((C, 2, 3)))
+
+
+def test_scatter_add_of_rank_gradients_equals_per_document_gradient():
+    """PAPER.md:109/204 + north_star invariance: sum over ranks of scatter_add(dk_r, dv_r) is the
+    gradient of running every document as its own causal attention (no sharding at all)."""
+    from oracle import attention as OA
+    rng = np.random.default_rng(5)
+    d, N, H, D = [24, 9, 15], 2, 2, 4
+    C = sum(d)
+    Q, K, V, dO = (rng.standard_normal((C, H, D)) for _ in range(4))
+    scale = 0.5
+    pl = P.plan(d, N)
+    dK, dV = np.zeros_like(K), np.zeros_like(V)
+    for r in range(N):
+        lay = KV.rank_layout(pl, r)
+        qi, gi = KV.q_token_index(pl, r), KV.gather_index(pl, r)
+        args = (lay.cu_seqlens_q, lay.q_pos_off, lay.shard_seg, lay.cu_seqlens_k, scale)
+        o, lse = OA.rank_fwd(Q[qi], K[gi], V[gi], *args)
+        _, dk, dv = OA.rank_bwd(Q[qi], K[gi], V[gi], o, lse, dO[qi], *args)
+        KV.scatter_add(pl, r, dk, dK)
+        KV.scatter_add(pl, r, dv, dV)
+    off = 0
+    for n in d:                                     # each document on its own: one shard, p = 0
+        one = (np.array([0, n]), np.array([0]), np.array([0]), np.array([0, n]), scale)
+        sl = slice(off, off + n)
+        o, lse = OA.rank_fwd(Q[sl], K[sl], V[sl], *one)
+        _, dk, dv = OA.rank_bwd(Q[sl], K[sl], V[sl], o, lse, dO[sl], *one)
+        assert np.abs(dK[sl] - dk).max() < 1e-12 and np.abs(dV[sl] - dv).max() < 1e-12
+        off += n

@@ -375,6 +375,26 @@ def run_fcp(args):
         gk_ms.append(t0.elapsed_time(t1) / 20)
         del ko, vo
     gather_gbs = sum(gather_bytes) / (sum(gk_ms) * 1e-3) / 1e9
+    # dKV scatter-add (not part of the timed step): same method.  Per token
+    # and tensor: bf16 source row + fp32 accumulator read + write = (2 + 4 + 4) * Hkv * D bytes.
+    sk_ms, scatter_bytes = [], []
+    dKg = torch.zeros((cfg.C, cfg.Hkv, cfg.D), dtype=torch.float32, device=dev)
+    dVg = torch.zeros_like(dKg)
+    for r in range(cfg.N):
+        dk_r = torch.zeros((w.n_kv[r], cfg.Hkv, cfg.D), dtype=torch.bfloat16, device=dev)
+        dv_r = torch.zeros_like(dk_r)
+        plan.kv_scatter_add(r, dk_r, dv_r, dKg, dVg)
+        torch.cuda.synchronize()
+        t0.record()
+        for _ in range(20):
+            plan.kv_scatter_add(r, dk_r, dv_r, dKg, dVg)
+        t1.record()
+        torch.cuda.synchronize()
+        sk_ms.append(t0.elapsed_time(t1) / 20)
+        scatter_bytes.append(2 * w.n_kv[r] * cfg.Hkv * cfg.D * 10)
+        del dk_r, dv_r
+    del dKg, dVg
+    scatter_gbs = sum(scatter_bytes) / (sum(sk_ms) * 1e-3) / 1e9
 
     # end to end from host buffers
     e2e = None
@@ -439,7 +459,11 @@ def run_fcp(args):
                 "kv_gather": {"gbs": gather_gbs, "frac_measured_hbm": gather_gbs / peaks["hbm"],
                               "kernel_ms_per_rank": gk_ms, "in_step_ms_per_rank_incl_host": g_ms,
                               "bytes_per_rank": gather_bytes,
-                              "how": "20 back-to-back launches per rank, CUDA events"}},
+                              "how": "20 back-to-back launches per rank, CUDA events"},
+                "kv_scatter_add": {"gbs": scatter_gbs, "frac_measured_hbm": scatter_gbs / peaks["hbm"],
+                                   "kernel_ms_per_rank": sk_ms, "bytes_per_rank": scatter_bytes,
+                                   "note": "dKV reduction stand-in (SURVEY 8(f) NEXT 1), bf16 source, "
+                                           "fp32 accumulators; outside the timed step"}},
             "plan": {"imbalance": st["imbalance_ppm"] / 1e6, "n_per_doc": st["n_per_doc"],
                      "max_load": st["max_load"], "mean_load": st["sum_load"] / cfg.N,
                      "eq4_kv_bytes": st["eq4_tokens"] * kv_b, "eq5_kv_bytes": st["eq5_tokens"] * kv_b,

@@ -130,6 +130,19 @@ int  fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, const void
                    void* k_out, void* v_out, int32_t n_kv_heads, int32_t head_dim,
                    void* stream, fcp_gather_counts* counts);
 
+/* dKV reduction of one rank (the gradients of the communicated KV go back to
+ * the ranks that own the tokens; the inverse of the KV selection of PAPER.md:111-113; SURVEY.md
+ * section 8(f) NEXT 1).  Adds the rank's own contribution dk_r, dv_r [n_kv, Hkv, D] (device,
+ * layout of the gathered k, v as written by fcp_attn_bwd; src_dtype FCP_DTYPE_BF16 or
+ * FCP_DTYPE_F32) into the global fp32 accumulators dK, dV [C, Hkv, D] (device): row i of the
+ * rank's buffer is added to global token kv_token_index[i].  The rows of one rank are distinct
+ * tokens, so one call needs no atomics; calls for different ranks must be ordered on the stream
+ * (virtual ranks) — across real GPUs this is the ReduceScatter the bytes of which *counts
+ * reports.  One kernel launch, asynchronous on `stream`. */
+int  fcp_kv_scatter_add(const fcp_plan* plan, int32_t rank, const void* dk_r, const void* dv_r,
+                        int32_t src_dtype, float* dK, float* dV, int32_t n_kv_heads,
+                        int32_t head_dim, void* stream, fcp_gather_counts* counts);
+
 /* ------------------------------------------------------------------------------------------
  * 3. Tile schedule of one rank: the (shard, q-tile, head) / (segment, kv-tile, kv-head) work
  *    lists of the attention kernels, ordered by descending cost so that short shards do not

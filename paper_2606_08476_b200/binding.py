@@ -12,7 +12,7 @@ LIB_PATH = os.path.join(_HERE, "libfcp.so")
 EXPORTS = [
     "fcp_strerror", "fcp_version", "fcp_plan_create", "fcp_plan_destroy", "fcp_plan_shards",
     "fcp_plan_perdoc", "fcp_plan_stats", "fcp_plan_rank_stats", "fcp_rank_layout",
-    "fcp_kv_gather", "fcp_sched_create", "fcp_sched_from_plan", "fcp_sched_destroy",
+    "fcp_kv_gather", "fcp_kv_scatter_add", "fcp_sched_create", "fcp_sched_from_plan", "fcp_sched_destroy",
     "fcp_sched_workspace_size", "fcp_sched_upload", "fcp_sched_get_info", "fcp_attn_fwd",
     "fcp_attn_bwd", "fcp_merge",
 ]
@@ -104,6 +104,9 @@ def _lib():
         lib.fcp_kv_gather.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
                                       C.POINTER(_GatherCounts)]
+        lib.fcp_kv_scatter_add.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32,
+                                           C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
+                                           C.c_void_p, C.POINTER(_GatherCounts)]
         lib.fcp_sched_create.argtypes = [_I32P, _I32P, _I32P, C.c_int32, _I32P, C.c_int32,
                                          C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
         lib.fcp_sched_from_plan.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
@@ -232,6 +235,23 @@ class Plan:
                                     v_out.data_ptr(), Hkv, D * K.element_size() // 2,
                                     _stream_ptr(stream), C.byref(cnt)), "fcp_kv_gather")
         return k_out, v_out, _struct_dict(cnt)
+
+    def kv_scatter_add(self, rank, dk_r, dv_r, dK, dV, stream=None):
+        """dK, dV (fp32 [C,Hkv,D]) += the rank's dk_r, dv_r (bf16 or fp32 [n_kv,Hkv,D], layout of
+        the gathered KV).  Returns the counts dict (bytes a ReduceScatter would move)."""
+        import torch
+        for t in (dk_r, dv_r, dK, dV):
+            assert t.is_cuda and t.is_contiguous()
+        assert dK.dtype == torch.float32 and dV.dtype == torch.float32
+        assert dk_r.dtype == dv_r.dtype and dk_r.dtype in (torch.bfloat16, torch.float32)
+        Hkv, D = dK.shape[1], dK.shape[2]
+        assert dk_r.shape[0] == self.rank_stats(rank)["n_kv"] and dk_r.shape[1:] == dK.shape[1:]
+        cnt = _GatherCounts()
+        _check(_lib().fcp_kv_scatter_add(self._h, rank, dk_r.data_ptr(), dv_r.data_ptr(),
+                                         0 if dk_r.dtype == torch.bfloat16 else 1, dK.data_ptr(),
+                                         dV.data_ptr(), Hkv, D, _stream_ptr(stream), C.byref(cnt)),
+               "fcp_kv_scatter_add")
+        return _struct_dict(cnt)
 
     def sched(self, rank, n_q_heads, n_kv_heads, head_dim):
         h = C.c_void_p()

@@ -128,6 +128,62 @@ template <> struct Vec8<float> {
   }
 };
 
+// ------------------------------------------------------------------------------------------
+// dKV scatter-add: the inverse of the gather.  dst (fp32, global token order) += src (bf16 or
+// fp32, gathered order) over the same contiguous ranges.  HBM-bound read-modify-write: per
+// element 2 or 4 B read + 4 B read + 4 B write.  One thread handles 8 consecutive elements
+// (16 B of bf16 / 32 B of fp32 in, 32 B in and out of the accumulator); all loads of a thread's
+// kScatterUnroll chunks are issued before its stores.
+// ------------------------------------------------------------------------------------------
+constexpr int kScatterThreads = 256;
+constexpr int kScatterUnroll = 4;
+
+template <typename T>
+__global__ void __launch_bounds__(kScatterThreads)
+fcp_kv_scatter_add_kernel(const T* __restrict__ dk_r, const T* __restrict__ dv_r,
+                          float* __restrict__ dK, float* __restrict__ dV,
+                          const __grid_constant__ GatherRanges rg) {
+  // rg is expressed in units of 8 elements: dst0 = offsets in the rank buffer, src0 = in dK/dV
+  const int64_t total = rg.dst0[rg.n];
+  constexpr int64_t kSpan = (int64_t)kScatterThreads * kScatterUnroll;
+  const int64_t n_spans = (total + kSpan - 1) / kSpan;
+  for (int64_t span = blockIdx.x; span < 2 * n_spans; span += gridDim.x) {
+    const bool is_v = span >= n_spans;
+    const int64_t c0 = (is_v ? span - n_spans : span) * kSpan;
+    const T* __restrict__ src = is_v ? dv_r : dk_r;
+    float* __restrict__ dst = is_v ? dV : dK;
+    int lo = 0, hi = rg.n - 1;                              // range that holds unit c0
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (rg.dst0[mid] <= c0) lo = mid; else hi = mid - 1;
+    }
+    float in[kScatterUnroll][8];
+    float4 acc[kScatterUnroll][2];
+    float4* where[kScatterUnroll];
+    int r = lo;
+#pragma unroll
+    for (int u = 0; u < kScatterUnroll; ++u) {
+      const int64_t c = c0 + u * kScatterThreads + threadIdx.x;
+      where[u] = nullptr;
+      if (c < total) {
+        while (c >= rg.dst0[r + 1]) ++r;
+        Vec8<T>::load(src, c, in[u]);
+        where[u] = reinterpret_cast<float4*>(dst) + 2 * (rg.src0[r] + (c - rg.dst0[r]));
+        acc[u][0] = where[u][0];
+        acc[u][1] = where[u][1];
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < kScatterUnroll; ++u)
+      if (where[u]) {
+        where[u][0] = make_float4(acc[u][0].x + in[u][0], acc[u][0].y + in[u][1],
+                                  acc[u][0].z + in[u][2], acc[u][0].w + in[u][3]);
+        where[u][1] = make_float4(acc[u][1].x + in[u][4], acc[u][1].y + in[u][5],
+                                  acc[u][1].z + in[u][6], acc[u][1].w + in[u][7]);
+      }
+  }
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256)
 fcp_merge_kernel(const void* __restrict__ o_a, const float* __restrict__ lse_a,
@@ -231,6 +287,70 @@ extern "C" int fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, 
         rg);
     if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
     dst_row += c / cpr;
+  }
+  return FCP_OK;
+}
+
+extern "C" int fcp_kv_scatter_add(const fcp_plan* plan, int32_t rank, const void* dk_r,
+                                  const void* dv_r, int32_t src_dtype, float* dK, float* dV,
+                                  int32_t n_kv_heads, int32_t head_dim, void* stream,
+                                  fcp_gather_counts* counts) {
+  if (!plan || rank < 0 || rank >= plan->n_ranks || !dk_r || !dv_r || !dK || !dV ||
+      n_kv_heads < 1 || head_dim < 1)
+    return FCP_INVALID_ARG;
+  if (src_dtype != FCP_DTYPE_BF16 && src_dtype != FCP_DTYPE_F32) return FCP_UNSUPPORTED;
+  const int64_t row_elems = (int64_t)n_kv_heads * head_dim;
+  if (row_elems % 8 != 0) return FCP_UNSUPPORTED;
+  if (!aligned16(dk_r) || !aligned16(dv_r) || !aligned16(dK) || !aligned16(dV)) return FCP_MISALIGNED;
+  RankView v;
+  fcp_build_rank_view(*plan, rank, v);
+  std::vector<int64_t> tok, len;                  // merged destination ranges (global tokens)
+  for (size_t g = 0; g < v.kv_len.size(); ++g) {
+    if (!tok.empty() && tok.back() + len.back() == v.kv_src_start[g]) {
+      len.back() += v.kv_len[g];
+    } else {
+      tok.push_back(v.kv_src_start[g]);
+      len.push_back(v.kv_len[g]);
+    }
+  }
+  const int64_t esz = src_dtype == FCP_DTYPE_F32 ? 4 : 2;
+  if (counts) {
+    counts->total_tokens = v.n_kv;
+    counts->remote_tokens = v.remote;
+    counts->total_bytes = 2 * v.n_kv * row_elems * esz;      // dk_r and dv_r, one pass
+    counts->remote_bytes = 2 * v.remote * row_elems * esz;   // what a ReduceScatter would move
+    counts->n_ranges = (int32_t)tok.size();
+    counts->reserved = 0;
+  }
+  const int64_t upr = row_elems / 8;              // 8-element units per row
+  int num_sms = 148, dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return FCP_CUDA;
+  cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+  int64_t src_row = 0;
+  for (size_t base = 0; base < tok.size(); base += kMaxRanges) {
+    GatherRanges rg;
+    std::memset(&rg, 0, sizeof(rg));
+    rg.n = (int32_t)std::min<size_t>(kMaxRanges, tok.size() - base);
+    int64_t c = 0;
+    for (int i = 0; i < rg.n; ++i) {
+      rg.dst0[i] = c;                             // position in the rank buffer
+      rg.src0[i] = tok[base + i] * upr;           // position in the global accumulator
+      c += len[base + i] * upr;
+    }
+    rg.dst0[rg.n] = c;
+    const int64_t spans = 2 * ((c + kScatterThreads * kScatterUnroll - 1) / (kScatterThreads * kScatterUnroll));
+    if (spans == 0) continue;
+    const int grid = (int)std::min<int64_t>(spans, (int64_t)num_sms * 8);
+    if (src_dtype == FCP_DTYPE_BF16)
+      fcp_kv_scatter_add_kernel<__nv_bfloat16><<<grid, kScatterThreads, 0, (cudaStream_t)stream>>>(
+          static_cast<const __nv_bfloat16*>(dk_r) + src_row * row_elems,
+          static_cast<const __nv_bfloat16*>(dv_r) + src_row * row_elems, dK, dV, rg);
+    else
+      fcp_kv_scatter_add_kernel<float><<<grid, kScatterThreads, 0, (cudaStream_t)stream>>>(
+          static_cast<const float*>(dk_r) + src_row * row_elems,
+          static_cast<const float*>(dv_r) + src_row * row_elems, dK, dV, rg);
+    if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
+    src_row += c / upr;
   }
   return FCP_OK;
 }

@@ -268,6 +268,48 @@ def test_plan_invariance_on_gpu(fcp, torch):
         U.check("dv", dv, want_dv)
 
 
+@pytest.mark.parametrize("src", ["bf16", "f32"])
+@pytest.mark.parametrize("name,strategy", [("tiny", 0), ("8b", 0), ("short", 0), ("8b", 1)],
+                         ids=["tiny", "8b", "short", "8b_all_per_doc"])
+def test_kv_scatter_add_matches_oracle(fcp, torch, name, strategy, src):
+    """fcp_kv_scatter_add against oracle.kvselect:
+    every virtual rank adds its dk_r, dv_r into the global fp32 accumulators; bf16 and fp32
+    sources convert exactly, one fp32 add per element and rank in rank order on both sides, so
+    the comparison is bit-exact against the same recurrence in fp32 (and within 1e-6 relative of
+    the fp64 oracle).  Tokens gathered by no rank must stay zero, which the oracle shows too."""
+    from oracle import kvselect as OKV, planner as OP
+    cfg = fcp_inputs.CONFIGS[name]
+    d = fcp_inputs.doc_lengths(name, 0)
+    Hkv, D = (cfg.Hkv, cfg.D) if name != "8b" else (2, 64)        # keep the 32K case light
+    plan = fcp.Plan(d, cfg.N, strategy=strategy)
+    pl = OP.plan(d, cfg.N, strategy=strategy)
+    gen = torch.Generator().manual_seed(11)
+    dK = torch.zeros((cfg.C, Hkv, D), dtype=torch.float32, device="cuda")
+    dV = torch.zeros_like(dK)
+    want_k = np.zeros((cfg.C, Hkv, D))
+    want_v = np.zeros_like(want_k)
+    f32_k = np.zeros((cfg.C, Hkv, D), dtype=np.float32)
+    total_remote = 0
+    for r in range(cfg.N):
+        n_kv = plan.rank_stats(r)["n_kv"]
+        dt = torch.bfloat16 if src == "bf16" else torch.float32
+        dk_r = torch.randn((n_kv, Hkv, D), generator=gen).to(dt)
+        dv_r = torch.randn((n_kv, Hkv, D), generator=gen).to(dt)
+        cnt = plan.kv_scatter_add(r, dk_r.cuda(), dv_r.cuda(), dK, dV)
+        assert cnt["total_tokens"] == n_kv and cnt["remote_tokens"] == plan.rank_stats(r)["remote_tokens"]
+        total_remote += cnt["remote_tokens"]
+        OKV.scatter_add(pl, r, U.to_f64(dk_r), want_k)
+        OKV.scatter_add(pl, r, U.to_f64(dv_r), want_v)
+        gi = OKV.gather_index(pl, r)
+        f32_k[gi] += dk_r.float().numpy()
+    torch.cuda.synchronize()
+    got_k, got_v = dK.cpu().numpy(), dV.cpu().numpy()
+    assert np.array_equal(got_k, f32_k)                                   # same fp32 recurrence
+    assert np.abs(got_k - want_k).max() <= 1e-6 * max(1.0, np.abs(want_k).max())
+    assert np.abs(got_v - want_v).max() <= 1e-6 * max(1.0, np.abs(want_v).max())
+    assert total_remote == plan.stats()["sum_remote_tokens"]
+
+
 def test_missing_library_fails_loudly(fcp, monkeypatch):
     import paper_2606_08476_b200.binding as B
     monkeypatch.setattr(B, "_LIB", None)

@@ -13,6 +13,7 @@ from typing import List, NamedTuple, Sequence
 STRATEGY_HYBRID = 0      # Algorithm 1
 STRATEGY_ALL_PER_DOC = 1  # every document Per-Doc
 STRATEGY_WHOLE_DOC = 2   # Whole-Doc only, never Per-Doc
+STRATEGY_PER_SEQ = 3     # Llama3 CP baseline: the packed SEQUENCE in 2N chunks
 
 DEFAULT_R_PPM = 1_050_000  # R = 1.05 (paper gives no value; its heuristic reaches 1.04)
 
@@ -52,12 +53,16 @@ def plan(d: Sequence[int], n_ranks: int, r_ppm: int = DEFAULT_R_PPM,
     n, N = len(d), int(n_ranks)
     if n < 1 or N < 1 or any(x < 1 for x in d) or r_ppm < 1_000_000:
         raise ValueError("invalid argument")
-    if strategy not in (STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC):
+    if strategy not in (STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC,
+                        STRATEGY_PER_SEQ):
         raise ValueError("invalid strategy")
     C = sum(d)
     if C % N != 0:                       # Eq. 2 needs C/N integral
         raise ValueError("C not divisible by N")
     T = C // N
+
+    if strategy == STRATEGY_PER_SEQ:
+        return _per_seq(d, N, C)
 
     # line 1: sort D in descending order of length (ties: lower id first)
     order = sorted(range(n), key=lambda k: (-d[k], k))
@@ -148,6 +153,41 @@ def plan(d: Sequence[int], n_ranks: int, r_ppm: int = DEFAULT_R_PPM,
         else:
             merged.append(s)
     return Plan(tuple(d), N, tuple(merged), tuple(order[:k_per]), tuple(pass_ratios))
+
+
+def _per_seq(d: List[int], N: int, C: int) -> Plan:
+    """Per-Sequence sharding, the Llama3 CP baseline the paper compares with (Fig.
+    1(b), Fig. 2): the packed sequence of C tokens is split into 2N equal chunks regardless of
+    document borders and worker i processes chunks i and 2N-1-i.  A chunk that spans several
+    documents yields one shard per document piece.  Needs C % 2N == 0 (equal chunks; reading
+    listed in DESIGN.md section 2.3).  No Per-Doc set, a single pass."""
+    if C % (2 * N) != 0:
+        raise ValueError("C not divisible by 2N")
+    q = C // (2 * N)
+    off = [0]
+    for x in d:
+        off.append(off[-1] + x)
+    shards = []
+    for c in range(2 * N):
+        j = c if c < N else 2 * N - 1 - c
+        lo, hi = c * q, (c + 1) * q
+        for k, x in enumerate(d):                       # pieces of documents inside [lo, hi)
+            a, b = max(lo, off[k]), min(hi, off[k + 1])
+            if a < b:
+                shards.append(Shard(k, a - off[k], b - a, j))
+    shards.sort(key=lambda s: (s.rank, s.doc, s.start))
+    merged: List[Shard] = []
+    for s in shards:
+        if merged and merged[-1].rank == s.rank and merged[-1].doc == s.doc \
+                and merged[-1].start + merged[-1].len == s.start:
+            last = merged.pop()
+            merged.append(Shard(s.doc, last.start, last.len + s.len, s.rank))
+        else:
+            merged.append(s)
+    load = [0] * N
+    for s in merged:
+        load[s.rank] += W(s.start, s.len)
+    return Plan(tuple(d), N, tuple(merged), (), ((max(load), sum(load)),))
 
 
 def rank_tokens(p: Plan) -> List[int]:

@@ -208,3 +208,56 @@ def test_invalid_arguments():
         P.plan([4, 4], 0)
     with pytest.raises(ValueError):
         P.plan([4, 4], 2, 999_999)
+
+
+# ---------------------------------------------------------------------------------------------
+# Per-Seq sharding (Llama3 CP baseline) — SURVEY 8(f) NEXT 3
+# ---------------------------------------------------------------------------------------------
+def test_per_seq_hand_worked_examples():
+    """Worked by hand from PAPER.md:50 ("split into 2 x CP shards, each worker processes two
+    shards"; chunks i and 2N-1-i as in PAPER.md:62).
+    D=[8,8], N=2: chunks of 4 tokens -> rank0 {[0,4) of doc0, [4,8) of doc1}, rank1 {[4,8) of
+    doc0, [0,4) of doc1}; W(0,4)=10, W(4,4)=26 -> loads 36/36.
+    D=[12,4], N=2: rank0 {doc0[0,4), doc1[0,4)} = 10+10, rank1 {doc0[4,12)} (chunks 1 and 2 are
+    contiguous and merge) = W(4,8) = 68 -> ratio 68*2/88 = 1.545 (the imbalance of Fig. 1(b))."""
+    pl = P.plan([8, 8], 2, strategy=P.STRATEGY_PER_SEQ)
+    assert pl.shards == (P.Shard(0, 0, 4, 0), P.Shard(1, 4, 4, 0), P.Shard(0, 4, 4, 1), P.Shard(1, 0, 4, 1))
+    assert P.rank_loads(pl) == [36, 36] and pl.per_doc == ()
+    pl = P.plan([12, 4], 2, strategy=P.STRATEGY_PER_SEQ)
+    assert pl.shards == (P.Shard(0, 0, 4, 0), P.Shard(1, 0, 4, 0), P.Shard(0, 4, 8, 1))
+    assert P.rank_loads(pl) == [20, 68]
+    assert P.imbalance_ppm(pl) == 68 * 2 * 1_000_000 // 88
+    with pytest.raises(ValueError):
+        P.plan([10, 4], 2, strategy=P.STRATEGY_PER_SEQ)      # C = 14 is not a multiple of 2N = 4
+
+
+def test_per_seq_invariants_and_single_document_equals_per_doc():
+    rng = np.random.default_rng(12)
+    for _ in range(60):
+        N = int(rng.integers(1, 6))
+        n = int(rng.integers(1, 7))
+        d = [int(x) for x in rng.integers(1, 40, size=n)]
+        pad = (-sum(d)) % (2 * N)
+        d[-1] += pad
+        pl = P.plan(d, N, strategy=P.STRATEGY_PER_SEQ)
+        C = sum(d)
+        # Eq. 1: every token of every document exactly once; Eq. 2: C/N tokens per worker
+        seen = [np.zeros(x, dtype=int) for x in d]
+        for s in pl.shards:
+            seen[s.doc][s.start:s.start + s.len] += 1
+        assert all((v == 1).all() for v in seen)
+        assert P.rank_tokens(pl) == [C // N] * N
+        assert sum(P.rank_loads(pl)) == sum(x * (x + 1) // 2 for x in d)
+        # chunk structure: worker j holds global tokens of chunks j and 2N-1-j only
+        q = C // (2 * N)
+        off = np.concatenate([[0], np.cumsum(d)])
+        for s in pl.shards:
+            g0, g1 = off[s.doc] + s.start, off[s.doc] + s.start + s.len - 1
+            for g in (g0, g1):
+                c = g // q
+                assert s.rank == (c if c < N else 2 * N - 1 - c)
+    # one document: Per-Seq is exactly all-Per-Doc (PAPER.md:62) when 2N divides it
+    for N in (1, 2, 4):
+        a = P.plan([16 * N], N, strategy=P.STRATEGY_PER_SEQ)
+        b = P.plan([16 * N], N, strategy=P.STRATEGY_ALL_PER_DOC)
+        assert a.shards == b.shards

@@ -49,7 +49,10 @@ typedef struct { int32_t doc, start, len, rank; } fcp_shard;
 
 enum { FCP_STRATEGY_HYBRID = 0,                 /* Algorithm 1: Whole-Doc + Per-Doc */
        FCP_STRATEGY_ALL_PER_DOC = 1,            /* every document in 2N chunks */
-       FCP_STRATEGY_WHOLE_DOC = 2 };            /* Whole-Doc sharding only */
+       FCP_STRATEGY_WHOLE_DOC = 2,              /* Whole-Doc sharding only */
+       FCP_STRATEGY_PER_SEQ = 3 };              /* baseline: Llama3 CP, the packed sequence in 2N
+                                                   chunks regardless of documents;
+                                                   needs C % 2N == 0 */
 
 typedef struct {
   int64_t imbalance_ppm;   /* target R = max/avg workload times 1e6; >= 1000000;

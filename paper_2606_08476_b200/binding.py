@@ -17,7 +17,7 @@ EXPORTS = [
     "fcp_attn_bwd", "fcp_merge",
 ]
 
-STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC = 0, 1, 2
+STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC, STRATEGY_PER_SEQ = 0, 1, 2, 3
 
 
 class FcpError(RuntimeError):

@@ -120,13 +120,14 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
     strategy = opts->strategy;
   }
   if (r_ppm < 1000000) return FCP_INVALID_ARG;
-  if (strategy < 0 || strategy > 2) return FCP_UNSUPPORTED;
+  if (strategy < 0 || strategy > FCP_STRATEGY_PER_SEQ) return FCP_UNSUPPORTED;
   int64_t C = 0;
   for (int i = 0; i < n_docs; ++i) {
     if (doc_lengths[i] < 1) return FCP_INVALID_ARG;
     C += doc_lengths[i];
   }
   if (C % n_ranks != 0 || C > INT32_MAX) return FCP_INVALID_ARG;
+  if (strategy == FCP_STRATEGY_PER_SEQ && C % (2 * (int64_t)n_ranks) != 0) return FCP_INVALID_ARG;
   const int N = n_ranks;
   const int64_t T = C / N;
 
@@ -138,6 +139,24 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
   for (int i = 0; i < n_docs; ++i) p->off[i + 1] = p->off[i] + p->d[i];
   p->n_ranks = N;  p->C = C;  p->T = T;
 
+  std::vector<fcp_shard> all;
+  if (strategy == FCP_STRATEGY_PER_SEQ) {
+    // Llama3 CP baseline: the packed sequence in 2N equal chunks regardless of
+    // document borders, chunks c and 2N-1-c on worker c; one shard per document piece.
+    const int64_t q = C / (2 * N);
+    int k = 0;
+    for (int c = 0; c < 2 * N; ++c) {
+      const int j = c < N ? c : 2 * N - 1 - c;
+      const int64_t lo = (int64_t)c * q, hi = lo + q;
+      while (p->off[k + 1] <= lo) ++k;
+      for (int kk = k; kk < n_docs && p->off[kk] < hi; ++kk) {
+        const int64_t a = std::max(lo, p->off[kk]), b = std::min(hi, p->off[kk + 1]);
+        if (a < b) all.push_back({kk, (int32_t)(a - p->off[kk]), (int32_t)(b - a), j});
+      }
+    }
+    p->n_passes = 1;
+  }
+
   std::vector<int32_t> order(n_docs);
   for (int i = 0; i < n_docs; ++i) order[i] = i;
   std::stable_sort(order.begin(), order.end(),
@@ -146,7 +165,7 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
   int k_per = strategy == FCP_STRATEGY_ALL_PER_DOC ? n_docs : 0;
   const int k_last = strategy == FCP_STRATEGY_WHOLE_DOC ? 0 : n_docs;
   Pass ps;
-  for (;;) {                                           // line 4
+  for (; strategy != FCP_STRATEGY_PER_SEQ;) {          // line 4
     run_pass(p->d, order, k_per, N, T, ps);
     ++p->n_passes;
     // Cur_R > R  <=>  max * N * 1e6 > R_ppm * sum, in 128 bits
@@ -155,13 +174,21 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
     if (!(lhs > rhs) || k_per >= k_last) break;
     ++k_per;                                           // lines 19-23
   }
-  p->per_doc.assign(order.begin(), order.begin() + k_per);
-  p->max_load = ps.max_load;
-  p->sum_load = ps.sum_load;
-
-  std::vector<fcp_shard> all(ps.chunks);
-  for (int j = 0; j < N; ++j)
-    for (const Item& it : ps.w[j].items) all.push_back({it.doc, it.start, it.len, j});
+  if (strategy != FCP_STRATEGY_PER_SEQ) {
+    p->per_doc.assign(order.begin(), order.begin() + k_per);
+    p->max_load = ps.max_load;
+    p->sum_load = ps.sum_load;
+    all = ps.chunks;
+    for (int j = 0; j < N; ++j)
+      for (const Item& it : ps.w[j].items) all.push_back({it.doc, it.start, it.len, j});
+  } else {
+    std::vector<uint64_t> load(N, 0);
+    for (const fcp_shard& s : all) load[s.rank] += fcp_W(s.start, s.len);
+    for (uint64_t x : load) {
+      p->max_load = std::max(p->max_load, x);
+      p->sum_load += x;
+    }
+  }
   std::sort(all.begin(), all.end(), [](const fcp_shard& a, const fcp_shard& b) {
     if (a.rank != b.rank) return a.rank < b.rank;
     if (a.doc != b.doc) return a.doc < b.doc;

@@ -102,6 +102,7 @@ CASES = [
     ([2048], 4, 8, 2, 128, 0),                     # one document, Per-Doc chunks, GQA 4
     ([33] * 31 + [1], 8, 2, 1, 64, 0),             # many short documents, shards < 64 rows
     ([1500, 400, 100, 48], 2, 2, 1, 128, 2),       # Whole-Doc head cut
+    ([900, 50, 700, 270, 128], 4, 4, 2, 128, 3),   # Per-Seq baseline plan: chunks cut documents anywhere
 ]
 
 

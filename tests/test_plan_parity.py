@@ -54,7 +54,7 @@ def test_bench_configs(fcp, name):
     for seed in (0, 1):
         d = fcp_inputs.doc_lengths(name, seed)
         assert sum(d) == cfg.C
-        for strategy in (0, 1, 2):
+        for strategy in (0, 1, 2, 3):
             assert_same_plan(fcp, d, cfg.N, 1_050_000, strategy)
 
 
@@ -80,3 +80,20 @@ def test_sched_info_counts_useful_pairs(fcp):
                     rows = min(128, b - a - r0)
                     fwd += (p + r0 + rows - 1) // 128 + 1
             assert info["fwd_kv_tiles"] == fwd * cfg.Hq
+
+
+def test_per_seq_random_and_errors(fcp):
+    """Per-Seq baseline plan (strategy 3): bit-exact plan, layout and statistics
+    against the oracle on random inputs; C % 2N != 0 is INVALID_ARG on both sides."""
+    rng = np.random.default_rng(21)
+    for _ in range(200):
+        N = int(rng.integers(1, 9))
+        n = int(rng.integers(1, 9))
+        d = [int(x) for x in rng.integers(1, 300, size=n)]
+        d[-1] += (-sum(d)) % (2 * N)
+        assert_same_plan(fcp, d, N, 1_050_000, 3)
+    with pytest.raises(fcp.FcpError) as e:
+        fcp.Plan([10, 4], 2, strategy=3)
+    assert e.value.status == -1
+    with pytest.raises(ValueError):
+        P.plan([10, 4], 2, strategy=3)

@@ -267,6 +267,53 @@ def hot_path_step(fcp, w, scale, ev=None, out=None):
     return plan
 
 
+def plan_compare(fcp, w, scale, reps=3):
+    """Relative comparison of sharding plans on the same kernels and the same packed batch (the
+    shape of the paper's Fig. 3 / Fig. 5): per strategy the critical path
+    max_r (fwd + bwd kernel time of virtual rank r), the sum over ranks, the load imbalance and
+    the KV bytes the plan would communicate.  Virtual ranks run one after another."""
+    import torch
+    cfg = w.cfg
+    names = {0: "flashcp_hybrid", 1: "all_per_doc", 2: "whole_doc_only", 3: "per_seq_llama3"}
+    Q = torch.empty((cfg.C, cfg.Hq, cfg.D), dtype=torch.bfloat16, device=w.K.device).normal_()
+    dO = torch.empty_like(Q).normal_()
+    kv_b = 2 * cfg.Hkv * cfg.D * 2
+    out = {}
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    for e in ev:
+        e.record()
+    for strategy, name in names.items():
+        try:
+            plan = fcp.Plan(w.d, cfg.N, strategy=strategy)
+        except fcp.FcpError:
+            continue
+        per_rank = []
+        for r in range(cfg.N):
+            qi = torch.from_numpy(plan.rank_layout(r)["q_token_index"].astype(np.int64)).to(Q.device)
+            q, do = Q[qi].contiguous(), dO[qi].contiguous()
+            sched = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload(Q.device)
+            kg, vg, _ = plan.kv_gather(r, w.K, w.V)
+            best = None
+            for _ in range(reps):
+                o, lse = sched.attn_fwd(q, kg, vg, scale, events=(ev[0], ev[1]))
+                sched.attn_bwd(q, kg, vg, o, lse, do, scale, events=(ev[2], ev[3]))
+                torch.cuda.synchronize()
+                t = ev[0].elapsed_time(ev[1]) + ev[2].elapsed_time(ev[3])
+                best = t if best is None else min(best, t)
+            per_rank.append(best)
+            del q, do, kg, vg, sched
+        st = plan.stats()
+        out[name] = {"critical_path_ms": max(per_rank), "sum_ms": sum(per_rank),
+                     "imbalance": st["imbalance_ppm"] / 1e6, "n_shards": st["n_shards"],
+                     "eq5_kv_bytes": st["eq5_tokens"] * kv_b,
+                     "max_remote_kv_bytes": st["max_remote_tokens"] * kv_b}
+    base = out.get("flashcp_hybrid", {}).get("critical_path_ms")
+    if base:
+        for v in out.values():
+            v["critical_path_vs_hybrid"] = v["critical_path_ms"] / base
+    return out
+
+
 def e2e_step(fcp, w, scale):
     """Same step from HOST buffers: pinned K, V, q, dO go host->device, results come back."""
     import torch
@@ -412,6 +459,8 @@ def run_fcp(args):
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": ems / args.steps}
 
+    compare = plan_compare(fcp, w, scale) if (args.plan_compare and rank == 0) else None
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = len(os.sched_getaffinity(0))
@@ -470,6 +519,8 @@ def run_fcp(args):
                      "max_remote_kv_bytes": st["max_remote_tokens"] * kv_b,
                      "sum_remote_kv_bytes": st["sum_remote_tokens"] * kv_b},
             "cpu_baseline": cpu}
+        if compare is not None:
+            line["plan_compare"] = compare
         print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
@@ -485,6 +536,8 @@ def main():
     ap.add_argument("--impl", default="fcp", choices=["fcp", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--plan-compare", action="store_true",
+                    help="also time hybrid / all-Per-Doc / Whole-Doc-only / Per-Seq plans on the same kernels")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -314,23 +314,48 @@ def plan_compare(fcp, w, scale, reps=3):
     return out
 
 
-def e2e_step(fcp, w, scale):
-    """Same step from HOST buffers: pinned K, V, q, dO go host->device, results come back."""
+def e2e_step(fcp, w, scale, streams):
+    """Same step from HOST buffers: pinned K, V, q, dO go host->device, results come back.
+    Three streams, as a user of the library would run it: uploads on `h2d` (K, V first, then every
+    virtual rank's q, dO), compute on the current stream as soon as a rank's inputs have landed,
+    downloads of o, dq, dk, dv on `d2h` behind the rank's backward — so PCIe runs in both
+    directions while the kernels run.  The current stream joins both at the end of the step."""
     import torch
     cfg = w.cfg
     dev = w.K.device
-    K, V = w.hK.to(dev, non_blocking=True), w.hV.to(dev, non_blocking=True)
+    cur = torch.cuda.current_stream()
+    h2d_s, d2h_s = streams
+    with torch.cuda.stream(h2d_s):     # not joined with the previous step: its downloads overlap these uploads
+        K, V = w.hK.to(dev, non_blocking=True), w.hV.to(dev, non_blocking=True)
+        ins = []
+        for r in range(cfg.N):
+            q, do = w.hq[r].to(dev, non_blocking=True), w.hdo[r].to(dev, non_blocking=True)
+            ev = torch.cuda.Event()
+            ev.record(h2d_s)
+            ins.append((q, do, ev))
     plan = fcp.Plan(w.d, cfg.N)
+    keep = [K, V]
     for r in range(cfg.N):
-        q, do = w.hq[r].to(dev, non_blocking=True), w.hdo[r].to(dev, non_blocking=True)
+        q, do, ev = ins[r]
         sched = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload(dev)
+        cur.wait_event(ev)                       # K, V and this rank's q, dO are on the device
         kg, vg, _ = plan.kv_gather(r, K, V)
         o, lse = sched.attn_fwd(q, kg, vg, scale)
         dq, dk, dv = sched.attn_bwd(q, kg, vg, o, lse, do, scale)
-        w.ho[r].copy_(o, non_blocking=True)
-        w.hdq[r].copy_(dq, non_blocking=True)
-        w.hdk[r].copy_(dk, non_blocking=True)
-        w.hdv[r].copy_(dv, non_blocking=True)
+        done = torch.cuda.Event()
+        done.record(cur)
+        d2h_s.wait_event(done)
+        with torch.cuda.stream(d2h_s):
+            w.ho[r].copy_(o, non_blocking=True)
+            w.hdq[r].copy_(dq, non_blocking=True)
+            w.hdk[r].copy_(dk, non_blocking=True)
+            w.hdv[r].copy_(dv, non_blocking=True)
+        keep += [q, do, kg, vg, o, lse, dq, dk, dv, sched]
+    cur.wait_stream(d2h_s)                       # the step ends when its results are on the host
+    for t in keep:                               # tensors used across streams: tell the allocator
+        if isinstance(t, torch.Tensor):
+            t.record_stream(cur)
+            t.record_stream(d2h_s)
     nb = lambda t: t.numel() * t.element_size()
     h2d = nb(w.hK) + nb(w.hV) + sum(nb(t) for t in w.hq) + sum(nb(t) for t in w.hdo)
     d2h = sum(nb(t) for t in w.ho + w.hdq + w.hdk + w.hdv)
@@ -446,12 +471,13 @@ def run_fcp(args):
     # end to end from host buffers
     e2e = None
     if not args.no_e2e:
+        side = (torch.cuda.Stream(), torch.cuda.Stream())
         for _ in range(2):
-            e2e_step(fcp, w, scale)
+            e2e_step(fcp, w, scale, side)
         barrier()
         t0.record()
         for _ in range(args.steps):
-            h2d, d2h = e2e_step(fcp, w, scale)
+            h2d, d2h = e2e_step(fcp, w, scale, side)
         t1.record()
         barrier()
         ems = max_over_ranks(t0.elapsed_time(t1))

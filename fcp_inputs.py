@@ -27,6 +27,11 @@ CONFIGS = {
     "longtail": Config("longtail", 131072, 8, 32, 8, 128),
     "short":    Config("short", 65536, 16, 32, 8, 128),
     "70b":      Config("70b", 262144, 8, 64, 8, 128),
+    # context-window sweep on the long-tail recipe (the shape of the paper's Fig. 7)
+    "longtail_64k":  Config("longtail_64k", 65536, 8, 32, 8, 128),
+    "longtail_256k": Config("longtail_256k", 262144, 8, 32, 8, 128),
+    "longtail_512k": Config("longtail_512k", 524288, 8, 32, 8, 128),
+    "longtail_1m":   Config("longtail_1m", 1048576, 8, 32, 8, 128),
     "fig3a":    Config("fig3a", 131072, 8, 32, 8, 128),
     "fig3b":    Config("fig3b", 131072, 8, 32, 8, 128),
 }
@@ -59,10 +64,10 @@ def doc_lengths(name: str, seed: int = 0) -> List[int]:
                                      128, 32768), C)
     if name == "short":
         return _fill(lambda: rng.integers(64, 1025), C)
-    if name == "longtail":
-        big = 73728
+    if name.startswith("longtail"):
+        big = C * 9 // 16                                    # 56 % of C (73728 at 128K)
         rest = _fill(lambda: np.clip(np.floor(256.0 * (1.0 - rng.random()) ** (-1.0 / 1.2)),
-                                     256, 131072), C - big)
+                                     256, C), C - big)
         pos = int(rng.integers(0, len(rest) + 1))
         return rest[:pos] + [big] + rest[pos:]
     if name == "70b":

@@ -345,18 +345,15 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       const int warp_min_limit = min(it.q_pos0 + (warp & 3) * 32, it.kv_len - 1);
       float m = -INFINITY, l = 0.f;
 
-      uint32_t sr[4][32];
-      bool prefetched = false;      // S_t(j) is already on its way into sr (issued in tile j-1)
       for (int j = 0; j < n; ++j) {
         if ((warp & 3) == 0) FTRACE(tn, 4 * t);
-        if (!prefetched) {
-          mbar_wait(&bars->s_full[t], s_ph);
-          tc_fence_after();
-#pragma unroll
-          for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, sr[c]);
-        }
+        mbar_wait(&bars->s_full[t], s_ph);
         if ((warp & 3) == 0) FTRACE(tn, 4 * t + 1);
         s_ph ^= 1;
+        tc_fence_after();
+        uint32_t sr[4][32];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, sr[c]);
         tmem_ld_wait();
         tc_fence_before();
         mbar_arrive(&bars->s_free[t]);              // S_t(j+1) may now overwrite S_t
@@ -474,15 +471,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tmem_st32(tO + c * 32, orow);
           }
           tmem_st_wait();
-        }
-        // S_t(j+1) was issued as soon as this tile's S sat in registers and is normally complete
-        // by now: start loading it before the hand-off so its latency overlaps the tail
-        prefetched = false;
-        if (j + 1 < n && __all_sync(0xffffffffu, mbar_test(&bars->s_full[t], s_ph))) {
-          tc_fence_after();
-#pragma unroll
-          for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, sr[c]);
-          prefetched = true;
         }
         fence_proxy_async_smem();
         tc_fence_before();

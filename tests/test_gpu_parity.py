@@ -311,6 +311,56 @@ def test_kv_scatter_add_matches_oracle(fcp, torch, name, strategy, src):
     assert total_remote == plan.stats()["sum_remote_tokens"]
 
 
+def test_outputs_do_not_write_out_of_bounds(fcp, torch):
+    """Canary rows around every output (o, lse, dq, dk, dv, gathered k/v) on ragged shapes whose
+    last tiles are partial: the kernels predicate their stores by q_rows / kv_rows and TMA boxes
+    run past shard ends, so a missing predicate shows up as a clobbered canary (this stands in
+    for a memory checker, which the pool does not offer)."""
+    d, N, Hq, Hkv, D = [333, 77, 130, 1, 63, 36], 2, 4, 2, 128
+    C = sum(d)
+    scale = 1.0 / math.sqrt(D)
+    Q, K, V, dO = fcp_inputs.make_tensors(C, Hq, Hkv, D, 9)
+    plan = fcp.Plan(d, N)
+    PAD, CAN = 70, 12345.0
+
+    def guarded(shape, dtype):
+        rows = shape[0] + 2 * PAD
+        buf = torch.full((rows,) + tuple(shape[1:]), CAN, dtype=dtype, device="cuda")
+        return buf, buf[PAD:PAD + shape[0]]
+
+    def intact(buf, n):
+        return bool((buf[:PAD] == CAN).all()) and bool((buf[PAD + n:] == CAN).all())
+
+    for r in range(N):
+        lay = plan.rank_layout(r)
+        qi = torch.from_numpy(lay["q_token_index"].astype(np.int64))
+        q, do = Q[qi].contiguous().cuda(), dO[qi].contiguous().cuda()
+        n_q, n_kv = q.shape[0], plan.rank_stats(r)["n_kv"]
+        kbuf, kg = guarded((n_kv, Hkv, D), torch.bfloat16)
+        vbuf, vg = guarded((n_kv, Hkv, D), torch.bfloat16)
+        plan.kv_gather(r, K.cuda(), V.cuda(), kg, vg)
+        sched = plan.sched(r, Hq, Hkv, D).upload("cuda")
+        obuf, o = guarded((n_q, Hq, D), torch.bfloat16)
+        # lse is [Hq, n_q]: guard it as one flat row-major block
+        lbuf = torch.full((Hq * n_q + 2 * PAD,), CAN, dtype=torch.float32, device="cuda")
+        lse = lbuf[PAD:PAD + Hq * n_q].view(Hq, n_q)
+        sched.attn_fwd(q, kg, vg, scale, o=o, lse=lse)
+        dqbuf, dq = guarded((n_q, Hq, D), torch.bfloat16)
+        dkbuf, dk = guarded((n_kv, Hkv, D), torch.bfloat16)
+        dvbuf, dv = guarded((n_kv, Hkv, D), torch.bfloat16)
+        sched.attn_bwd(q, kg, vg, o, lse, do, scale, dq=dq, dk=dk, dv=dv)
+        torch.cuda.synchronize()
+        assert intact(kbuf, n_kv) and intact(vbuf, n_kv), "gather wrote outside k_out / v_out"
+        assert intact(obuf, n_q), "fwd wrote outside o"
+        assert bool((lbuf[:PAD] == CAN).all()) and bool((lbuf[PAD + Hq * n_q:] == CAN).all()), "fwd wrote outside lse"
+        assert intact(dqbuf, n_q), "bwd wrote outside dq"
+        assert intact(dkbuf, n_kv) and intact(dvbuf, n_kv), "bwd wrote outside dk / dv"
+        # and everything inside was written (no canary left)
+        for t in (o, dq, dk, dv, kg, vg):
+            assert not bool((t == CAN).any())
+        assert not bool((lse == CAN).any())
+
+
 def test_missing_library_fails_loudly(fcp, monkeypatch):
     import paper_2606_08476_b200.binding as B
     monkeypatch.setattr(B, "_LIB", None)

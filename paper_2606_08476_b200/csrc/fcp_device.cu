@@ -380,20 +380,10 @@ extern "C" int fcp_merge(const void* o_a, const float* lse_a, const void* o_b, c
 extern "C" int fcp_sched_upload(const fcp_sched* s, void* workspace, void* stream) {
   if (!s || !workspace) return FCP_INVALID_ARG;
   if (!aligned16(workspace)) return FCP_MISALIGNED;
-  char* w = static_cast<char*>(workspace);
-  cudaStream_t st = (cudaStream_t)stream;
-  auto put = [&](size_t off, const void* src, size_t bytes) {
-    return bytes == 0 ||
-           cudaMemcpyAsync(w + off, src, bytes, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  };
-  bool ok = cudaMemsetAsync(w + s->off_counters, 0, 256, st) == cudaSuccess;
-  ok = ok && put(s->off_fwd, s->fwd.data(), s->fwd.size() * sizeof(FwdItem));
-  ok = ok && put(s->off_bwd, s->bwd.data(), s->bwd.size() * sizeof(BwdItem));
-  ok = ok && put(s->off_sub, s->bwd_sub.data(), s->bwd_sub.size() * sizeof(BwdSub));
-  ok = ok && put(s->off_fwd_cta, s->fwd_cta_off.data(), s->fwd_cta_off.size() * sizeof(int32_t));
-  ok = ok && put(s->off_bwd_cta, s->bwd_cta_off.data(), s->bwd_cta_off.size() * sizeof(int32_t));
-  ok = ok && put(s->off_shard_meta, s->tile_meta.data(), s->tile_meta.size() * sizeof(int32_t));
-  // The sources are pageable host vectors owned by the schedule: cudaMemcpyAsync returns once
-  // they are staged, so no synchronisation is needed here.
+  // The lists were laid out in one host image by fcp_sched_create: a single copy.  The source
+  // is pageable host memory owned by the schedule: cudaMemcpyAsync returns once it is staged,
+  // so no synchronisation is needed here.
+  const bool ok = cudaMemcpyAsync(workspace, s->image.data(), s->image.size(), cudaMemcpyHostToDevice,
+                                  (cudaStream_t)stream) == cudaSuccess;
   return ok ? FCP_OK : FCP_CUDA;
 }

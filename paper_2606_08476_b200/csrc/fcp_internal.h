@@ -74,6 +74,7 @@ struct fcp_sched {
   std::vector<FwdItem> fwd;
   std::vector<BwdItem> bwd;
   std::vector<int32_t> fwd_cta_off, bwd_cta_off;   // [n_cta + 1]
+  std::vector<uint8_t> image;                      // host image of workspace [0, off_lsed): one upload
   std::vector<BwdSub> bwd_sub;
   int64_t fwd_kv_tiles = 0, bwd_tile_pairs = 0;
   uint64_t useful_pairs = 0;

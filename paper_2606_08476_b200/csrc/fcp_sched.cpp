@@ -6,6 +6,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cstring>
 #include <new>
 #include <queue>
 
@@ -179,6 +180,18 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
   s->off_lsed = o;      o = align_up(o + (size_t)s->Hq * s->n_q_pad * 2 * sizeof(float), 256);
   s->off_dq = o;        o = align_up(o + (size_t)s->n_q_pad * s->Hq * s->D * sizeof(float), 256);
   s->total = std::max<size_t>(o, 256);
+  // host image of the list part of the workspace, uploaded with ONE copy (the per-rank host
+  // latency matters on batches of short documents)
+  s->image.assign(s->off_lsed, 0);
+  auto put = [&](size_t off, const void* src, size_t bytes) {
+    if (bytes) std::memcpy(s->image.data() + off, src, bytes);
+  };
+  put(s->off_fwd, s->fwd.data(), s->fwd.size() * sizeof(FwdItem));
+  put(s->off_bwd, s->bwd.data(), s->bwd.size() * sizeof(BwdItem));
+  put(s->off_sub, s->bwd_sub.data(), s->bwd_sub.size() * sizeof(BwdSub));
+  put(s->off_fwd_cta, s->fwd_cta_off.data(), s->fwd_cta_off.size() * sizeof(int32_t));
+  put(s->off_bwd_cta, s->bwd_cta_off.data(), s->bwd_cta_off.size() * sizeof(int32_t));
+  put(s->off_shard_meta, s->tile_meta.data(), s->tile_meta.size() * sizeof(int32_t));
   *out = s;
   return FCP_OK;
 }

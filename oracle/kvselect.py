@@ -138,3 +138,64 @@ def scatter_add(p: Plan, rank: int, dkv_rank: np.ndarray, dKV_global: np.ndarray
         raise ValueError("dkv_rank has %d rows, the rank gathers %d" % (dkv_rank.shape[0], gi.shape[0]))
     # the gathered rows of one rank are distinct tokens, so a plain indexed add is exact
     dKV_global[gi] += dkv_rank
+
+
+# ---------------------------------------------------------------------------------------------
+# Local / prefix split of a rank's keys.
+#
+# PAPER.md:15 and PAPER.md:234 describe the communication-hiding alternative FlashCP is compared
+# with: compute on the keys a worker already holds while the others travel, then aggregate the
+# partial results.  The split used here is per shard (k, p, s) of the rank:
+#   LOCAL  piece: the shard's own tokens  [p, p+s)   — causal inside the shard;
+#   PREFIX piece: the tokens before it    [0, p)     — every key visible to every row.
+# The two key sets are disjoint and their union is the prefix [0, p+s) the row-wise definition
+# needs, so merging the two partial attentions (attention.merge) gives exactly
+# the unsplit result.  Each shard is its own KV segment in both pieces; a prefix that another
+# shard of the same rank also needs appears once per shard in the PREFIX buffer.
+# ---------------------------------------------------------------------------------------------
+PIECE_LOCAL = 1
+PIECE_PREFIX = 2
+
+
+def piece_layout(p: Plan, rank: int, piece: int) -> RankLayout:
+    """Varlen descriptors of one piece: one KV segment per shard of the rank (seg_doc = the
+    shard's document); q_pos_off is relative to the segment's first key."""
+    if piece not in (PIECE_LOCAL, PIECE_PREFIX):
+        raise ValueError("piece")
+    off = doc_offsets(p.d)
+    cu_q, ppos, sseg, cu_k, kv_src, kv_len, seg_doc = [0], [], [], [0], [], [], []
+    for s in p.shards:
+        if s.rank != rank:
+            continue
+        cu_q.append(cu_q[-1] + s.len)
+        sseg.append(len(kv_src))
+        if piece == PIECE_LOCAL:
+            ppos.append(0)                         # row t sees keys 0..t of its own shard
+            kv_src.append(off[s.doc] + s.start)
+            kv_len.append(s.len)
+        else:
+            ppos.append(s.start)                   # row t sees keys j <= p + t, all j < p
+            kv_src.append(off[s.doc])
+            kv_len.append(s.start)
+        seg_doc.append(s.doc)
+        cu_k.append(cu_k[-1] + kv_len[-1])
+    i32 = lambda a: np.asarray(a, dtype=np.int32)
+    return RankLayout(i32(cu_q), i32(ppos), i32(sseg), i32(cu_k), i32(kv_src), i32(kv_len),
+                      i32(seg_doc))
+
+
+def piece_gather_index(p: Plan, rank: int, piece: int) -> np.ndarray:
+    """Global token index of every row of the piece's KV buffer, int32."""
+    L = piece_layout(p, rank, piece)
+    out = []
+    for a, n in zip(L.kv_src_start, L.kv_len):
+        out.extend(range(int(a), int(a) + int(n)))
+    return np.asarray(out, dtype=np.int32)
+
+
+def piece_remote_tokens(p: Plan, rank: int, piece: int) -> int:
+    """Distinct tokens of the piece's buffer that another rank owns: what a CP group would have
+    to deliver before the piece can run (0 for LOCAL; for PREFIX the same tokens as the unsplit
+    gather's remote part, each counted once however many shards repeat it)."""
+    idx = np.unique(piece_gather_index(p, rank, piece))
+    return int((owner_of_tokens(p)[idx] != rank).sum()) if idx.size else 0

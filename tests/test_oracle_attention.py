@@ -247,3 +247,45 @@ def test_sampled_rows_match_full():
     so, sl = A.shard_rows_fwd(q[rows], k, v, p + rows + 1, scale)
     np.testing.assert_allclose(so, o[rows], atol=1e-13)
     np.testing.assert_allclose(sl, lse[:, rows], atol=1e-13)
+
+
+def test_local_prefix_split_merges_to_the_packed_result():
+    """attention over the LOCAL and the PREFIX piece of every rank, merged
+    (PAPER.md:64, 234), equals the plain packed definition — forward and, with the
+    merged o / lse, backward (dq adds over the pieces, dK / dV scatter-add)."""
+    rng = np.random.default_rng(15)
+    Hq, Hkv, D, scale = 4, 2, 8, 0.3
+    for trial in range(6):
+        N = int(rng.integers(1, 5))
+        d = [int(x) for x in rng.integers(1, 70, size=int(rng.integers(1, 6)))]
+        pad = (-sum(d)) % N
+        if pad:
+            d.append(pad)
+        C = sum(d)
+        Q, K, V, dO = rnd(rng, C, Hq, D), rnd(rng, C, Hkv, D), rnd(rng, C, Hkv, D), rnd(rng, C, Hq, D)
+        want_o, want_lse = A.packed_fwd(Q, K, V, d, scale)
+        want_dq, want_dk, want_dv = A.packed_bwd(Q, K, V, dO, d, scale)
+        for strategy in (0, 1):
+            pl = P.plan(d, N, 1_050_000, strategy)
+            o, lse = np.zeros_like(Q), np.zeros((Hq, C))
+            dq, dk, dv = np.zeros_like(Q), np.zeros_like(K), np.zeros_like(V)
+            for r in range(N):
+                qi = KV.q_token_index(pl, r)
+                part = {}
+                for piece in (KV.PIECE_LOCAL, KV.PIECE_PREFIX):
+                    L = KV.piece_layout(pl, r, piece)
+                    gi = KV.piece_gather_index(pl, r, piece)
+                    part[piece] = (L, gi) + A.rank_fwd(Q[qi], K[gi], V[gi], L.cu_seqlens_q,
+                                                       L.q_pos_off, L.shard_seg, L.cu_seqlens_k, scale)
+                o_r, lse_r = A.merge(*part[KV.PIECE_LOCAL][2:], *part[KV.PIECE_PREFIX][2:])
+                o[qi], lse[:, qi] = o_r, lse_r
+                for piece in (KV.PIECE_LOCAL, KV.PIECE_PREFIX):
+                    L, gi = part[piece][:2]
+                    dq_p, dk_p, dv_p = A.rank_bwd(Q[qi], K[gi], V[gi], o_r, lse_r, dO[qi],
+                                                  L.cu_seqlens_q, L.q_pos_off, L.shard_seg,
+                                                  L.cu_seqlens_k, scale)
+                    dq[qi] += dq_p
+                    np.add.at(dk, gi, dk_p)
+                    np.add.at(dv, gi, dv_p)
+            for g, w in zip((o, lse, dq, dk, dv), (want_o, want_lse, want_dq, want_dk, want_dv)):
+                np.testing.assert_allclose(g, w, atol=1e-11)

@@ -134,3 +134,72 @@ def test_scatter_add_of_rank_gradients_equals_per_document_gradient():
         _, dk, dv = OA.rank_bwd(Q[sl], K[sl], V[sl], o, lse, dO[sl], *one)
         assert np.abs(dK[sl] - dk).max() < 1e-12 and np.abs(dV[sl] - dv).max() < 1e-12
         off += n
+
+
+# ------------------------------------------------------------------ local / prefix split
+def visible_pairs_bruteforce(pl, rank):
+    """{(global query token, global key token)} of one rank, pair by pair from the document
+    mask (PAPER.md:46)."""
+    off = KV.doc_offsets(pl.d)
+    pairs = set()
+    for s in pl.shards:
+        if s.rank == rank:
+            for t in range(s.start, s.start + s.len):
+                for j in range(t + 1):
+                    pairs.add((off[s.doc] + t, off[s.doc] + j))
+    return pairs
+
+
+def piece_pairs(pl, rank, piece):
+    """(query, key) pairs a piece computes, read off its varlen descriptors with the layout rule
+    of include/fcp.h: row t of shard i sees key j of its segment iff j <= q_pos_off + t, j < len."""
+    L = KV.piece_layout(pl, rank, piece)
+    qi = KV.q_token_index(pl, rank)
+    gi = KV.piece_gather_index(pl, rank, piece)
+    pairs = []
+    for i in range(len(L.q_pos_off)):
+        g = int(L.shard_seg[i])
+        k0, k1 = int(L.cu_seqlens_k[g]), int(L.cu_seqlens_k[g + 1])
+        for t in range(int(L.cu_seqlens_q[i + 1] - L.cu_seqlens_q[i])):
+            for j in range(min(k1 - k0, int(L.q_pos_off[i]) + t + 1)):
+                pairs.append((int(qi[L.cu_seqlens_q[i] + t]), int(gi[k0 + j])))
+    return pairs
+
+
+def test_local_and_prefix_pieces_partition_the_visible_pairs():
+    for d, N, r_ppm, strategy in random_inputs(11, 60):
+        pl = P.plan(d, N, r_ppm, strategy)
+        for r in range(N):
+            loc = piece_pairs(pl, r, KV.PIECE_LOCAL)
+            pre = piece_pairs(pl, r, KV.PIECE_PREFIX)
+            assert len(set(loc)) == len(loc) and len(set(pre)) == len(pre)   # nothing twice
+            assert not (set(loc) & set(pre))                                 # disjoint
+            assert set(loc) | set(pre) == visible_pairs_bruteforce(pl, r)    # complete
+            # LOCAL needs nothing from other ranks; PREFIX needs what the unsplit gather needs
+            assert list(KV.piece_gather_index(pl, r, KV.PIECE_LOCAL)) == list(KV.q_token_index(pl, r))
+            assert KV.piece_remote_tokens(pl, r, KV.PIECE_LOCAL) == 0
+            assert KV.piece_remote_tokens(pl, r, KV.PIECE_PREFIX) == KV.kv_stats(pl).remote[r]
+            # the pair counts are the two terms of W(p, s) = s(s+1)/2 + p s  (PAPER.md:74)
+            mine = [s for s in pl.shards if s.rank == r]
+            assert len(loc) == sum(s.len * (s.len + 1) // 2 for s in mine)
+            assert len(pre) == sum(s.start * s.len for s in mine)
+
+
+def test_piece_layout_worked_example():
+    # d = (8, 4), N = 2, all Per-Doc (chunks of 2 and 1): rank 0 holds doc0 [0,2)+[6,8) and
+    # doc1 [0,1)+[3,4); rank 1 holds doc0 [2,6) and doc1 [1,3)
+    pl = P.plan([8, 4], 2, 1_000_000, P.STRATEGY_ALL_PER_DOC)
+    assert [(s.doc, s.start, s.len) for s in pl.shards if s.rank == 0] == \
+        [(0, 0, 2), (0, 6, 2), (1, 0, 1), (1, 3, 1)]
+    loc = KV.piece_layout(pl, 0, KV.PIECE_LOCAL)
+    assert list(loc.cu_seqlens_k) == [0, 2, 4, 5, 6] and list(loc.q_pos_off) == [0, 0, 0, 0]
+    assert list(loc.kv_src_start) == [0, 6, 8, 11]
+    pre = KV.piece_layout(pl, 0, KV.PIECE_PREFIX)
+    assert list(pre.kv_len) == [0, 6, 0, 3] and list(pre.q_pos_off) == [0, 6, 0, 3]
+    assert list(pre.kv_src_start) == [0, 0, 8, 8] and list(pre.cu_seqlens_k) == [0, 0, 6, 6, 9]
+    assert list(KV.piece_gather_index(pl, 0, KV.PIECE_PREFIX)) == [0, 1, 2, 3, 4, 5, 8, 9, 10]
+    assert KV.piece_remote_tokens(pl, 0, KV.PIECE_PREFIX) == 4 + 2      # doc0 [2,6), doc1 [1,3)
+    one = KV.piece_layout(pl, 1, KV.PIECE_PREFIX)
+    assert list(one.kv_len) == [2, 1] and list(one.shard_seg) == [0, 1]
+    with pytest.raises(ValueError):
+        KV.piece_layout(pl, 0, 0)

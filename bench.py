@@ -314,6 +314,59 @@ def plan_compare(fcp, w, scale, reps=3):
     return out
 
 
+def split_compare(fcp, w, scale, reps=3):
+    """Local / prefix split (include/fcp.h section 2b)
+    against the unsplit path on the same batch and kernels.  Per virtual rank, device time of
+      unsplit: gather + fwd | bwd
+      split  : LOCAL gather + fwd (needs no remote byte) | PREFIX gather + fwd | merge |
+               bwd LOCAL + bwd PREFIX sharing the fp32 dq accumulator
+    summed over the ranks (best of `reps`).  `local_share_of_fwd` is the part of the split
+    forward that can run before any remote KV has arrived — the time an exchange could hide
+    behind; `fwd_overhead` / `bwd_overhead` is what the split costs in kernel time."""
+    import torch
+    cfg = w.cfg
+    plan = fcp.Plan(w.d, cfg.N)
+    keys = ("unsplit_fwd", "unsplit_bwd", "local_fwd", "prefix_fwd", "merge", "split_bwd")
+    tot = dict.fromkeys(keys, 0.0)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(7)]
+    for r in range(cfg.N):
+        q, do = w.q[r], w.do[r]
+        sf = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload(q.device)
+        sl = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D, fcp.PIECE_LOCAL).upload(q.device)
+        sp = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D, fcp.PIECE_PREFIX).upload(q.device)
+        acc = sl.dq_accumulator(q.device)
+        best = dict.fromkeys(keys, float("inf"))
+        for _ in range(reps):
+            ev[0].record()
+            kg, vg, _ = plan.kv_gather(r, w.K, w.V)
+            o, lse = sf.attn_fwd(q, kg, vg, scale)
+            ev[1].record()
+            sf.attn_bwd(q, kg, vg, o, lse, do, scale)
+            ev[2].record()
+            kl, vl, _ = plan.kv_gather(r, w.K, w.V, piece=fcp.PIECE_LOCAL)
+            ol, ll = sl.attn_fwd(q, kl, vl, scale)
+            ev[3].record()
+            kp, vp, _ = plan.kv_gather(r, w.K, w.V, piece=fcp.PIECE_PREFIX)
+            op, lp = sp.attn_fwd(q, kp, vp, scale)
+            ev[4].record()
+            om, lm = fcp.merge(ol, ll, op, lp)
+            ev[5].record()
+            sl.attn_bwd(q, kl, vl, om, lm, do, scale, dq_accum=acc, dq_flags=fcp.DQ_NO_OUTPUT)
+            sp.attn_bwd(q, kp, vp, om, lm, do, scale, dq_accum=acc, dq_flags=fcp.DQ_KEEP)
+            ev[6].record()
+            torch.cuda.synchronize()
+            for i, k in enumerate(keys):
+                best[k] = min(best[k], ev[i].elapsed_time(ev[i + 1]))
+            del kg, vg, kl, vl, kp, vp
+        for k in keys:
+            tot[k] += best[k]
+    split_fwd = tot["local_fwd"] + tot["prefix_fwd"] + tot["merge"]
+    return {"ms_sum_over_ranks": {k: round(v, 4) for k, v in tot.items()},
+            "fwd_overhead": split_fwd / tot["unsplit_fwd"],
+            "bwd_overhead": tot["split_bwd"] / tot["unsplit_bwd"],
+            "local_share_of_fwd": tot["local_fwd"] / split_fwd}
+
+
 def e2e_step(fcp, w, scale, streams):
     """Same step from HOST buffers: pinned K, V, q, dO go host->device, results come back.
     Three streams, as a user of the library would run it: uploads on `h2d` (K, V first, then every
@@ -486,6 +539,7 @@ def run_fcp(args):
                "ms_per_step": ems / args.steps}
 
     compare = plan_compare(fcp, w, scale) if (args.plan_compare and rank == 0) else None
+    split = split_compare(fcp, w, scale) if (args.split_compare and rank == 0) else None
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -547,6 +601,8 @@ def run_fcp(args):
             "cpu_baseline": cpu}
         if compare is not None:
             line["plan_compare"] = compare
+        if split is not None:
+            line["split_compare"] = split
         print(json.dumps(line))
     if dist:
         dist.destroy_process_group()
@@ -564,6 +620,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--plan-compare", action="store_true",
                     help="also time hybrid / all-Per-Doc / Whole-Doc-only / Per-Seq plans on the same kernels")
+    ap.add_argument("--split-compare", action="store_true",
+                    help="also time the local / prefix split of every rank's keys against the unsplit path")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

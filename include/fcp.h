@@ -147,6 +147,38 @@ int  fcp_kv_scatter_add(const fcp_plan* plan, int32_t rank, const void* dk_r, co
                         int32_t head_dim, void* stream, fcp_gather_counts* counts);
 
 /* ------------------------------------------------------------------------------------------
+ * 2b. Local / prefix split of a rank's keys.  PAPER.md:15 and
+ *    PAPER.md:234 describe the communication-hiding alternative: compute on the keys a worker
+ *    already holds while the others travel, then aggregate the partial results.
+ *    Per shard (k, p, s) of the rank:
+ *      FCP_PIECE_LOCAL  : the shard's own tokens [p, p+s), causal inside the shard — needs no
+ *                         byte from another rank (its buffer is the rank's own K/V rows in
+ *                         local query order);
+ *      FCP_PIECE_PREFIX : the tokens [0, p) before it, all visible to every row.
+ *    The two key sets are disjoint and their union is the prefix [0, p+s) the unsplit path
+ *    (FCP_PIECE_FULL) attends to, so  fcp_merge(fwd(LOCAL), fwd(PREFIX))  equals the unsplit
+ *    forward; the backward of each piece takes the merged o / lse, dq accumulates over the
+ *    pieces (fcp_attn_args.dq_accum) and dK / dV scatter-add per piece.
+ *    In both pieces every shard is its own KV segment (n_segs = n_shards, zero-length segments
+ *    allowed); a prefix two shards of the rank share appears once per shard in the PREFIX
+ *    buffer, and fcp_rank_stats.remote_tokens / counts->remote_* still count each distinct
+ *    remote token once (LOCAL: 0, PREFIX: the unsplit gather's).  The *_piece entry points with
+ *    FCP_PIECE_FULL are the plain ones.
+ * ------------------------------------------------------------------------------------------ */
+enum { FCP_PIECE_FULL = 0, FCP_PIECE_LOCAL = 1, FCP_PIECE_PREFIX = 2 };
+int  fcp_plan_piece_stats(const fcp_plan* plan, int32_t rank, int32_t piece, fcp_rank_stats* out);
+int  fcp_piece_layout(const fcp_plan* plan, int32_t rank, int32_t piece, fcp_layout* out);
+int  fcp_kv_gather_piece(const fcp_plan* plan, int32_t rank, int32_t piece, const void* K,
+                         const void* V, void* k_out, void* v_out, int32_t n_kv_heads,
+                         int32_t head_dim, void* stream, fcp_gather_counts* counts);
+/* Rows of a PREFIX buffer can name the same global token twice (two shards of one document on
+ * the rank); such ranges are added by separate, stream-ordered launches — still no atomics. */
+int  fcp_kv_scatter_add_piece(const fcp_plan* plan, int32_t rank, int32_t piece, const void* dk_r,
+                              const void* dv_r, int32_t src_dtype, float* dK, float* dV,
+                              int32_t n_kv_heads, int32_t head_dim, void* stream,
+                              fcp_gather_counts* counts);
+
+/* ------------------------------------------------------------------------------------------
  * 3. Tile schedule of one rank: the (shard, q-tile, head) / (segment, kv-tile, kv-head) work
  *    lists of the attention kernels, ordered by descending cost so that short shards do not
  *    starve the SMs.  Host object; fcp_sched_upload copies the lists into
@@ -164,6 +196,9 @@ int  fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
                       fcp_sched** out);          /* all arrays host */
 int  fcp_sched_from_plan(const fcp_plan* plan, int32_t rank, int32_t n_q_heads,
                          int32_t n_kv_heads, int32_t head_dim, fcp_sched** out);
+int  fcp_sched_from_plan_piece(const fcp_plan* plan, int32_t rank, int32_t piece,
+                               int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                               fcp_sched** out);             /* section 2b */
 void fcp_sched_destroy(fcp_sched* sched);
 /* Device bytes needed by fcp_sched_upload + fcp_attn_fwd + fcp_attn_bwd (work lists, tile
  * counters, backward scratch: padded (lse, delta) and the fp32 dq accumulator). */
@@ -176,6 +211,8 @@ typedef struct {
   int64_t bwd_tile_pairs;             /* (kv-tile, q-tile) pairs the backward computes, x heads */
   uint64_t useful_pairs;              /* sum of unmasked (q,k) pairs over the rank's shards */
   int64_t n_q, n_kv;
+  int64_t n_q_pad;                    /* query rows with every shard padded to a multiple of the
+                                         backward's q tile: rows of fcp_attn_args.dq_accum */
 } fcp_sched_info;
 int  fcp_sched_get_info(const fcp_sched* sched, fcp_sched_info* out);
 
@@ -205,7 +242,16 @@ typedef struct {
   void*       ev_stop;       /* ... and right after the call's dominant kernel (the tcgen05
                                 attention kernel of fwd / the main kernel of bwd): lets a caller
                                 time that kernel alone without a profiler */
+  float*      dq_accum;      /* fcp_attn_bwd only, optional (NULL = the workspace's own): device
+                                f32 [Hq, n_q_pad, D] accumulator of UNSCALED dQ shared by the
+                                backward calls over several KV pieces of the same queries
+                                (section 2b; the pieces' schedules have the same n_q_pad) */
+  int32_t     dq_flags;      /* FCP_DQ_* bits, only read when dq_accum != NULL */
 } fcp_attn_args;
+enum {
+  FCP_DQ_KEEP = 1,           /* do not zero dq_accum first: it holds an earlier piece's partial */
+  FCP_DQ_NO_OUTPUT = 2       /* do not convert to dq yet (dq may be NULL): more pieces follow */
+};
 int  fcp_attn_fwd(const fcp_attn_args* args);
 int  fcp_attn_bwd(const fcp_attn_args* args, const void* dO, void* dq, void* dk, void* dv);
 

@@ -14,10 +14,14 @@ EXPORTS = [
     "fcp_plan_perdoc", "fcp_plan_stats", "fcp_plan_rank_stats", "fcp_rank_layout",
     "fcp_kv_gather", "fcp_kv_scatter_add", "fcp_sched_create", "fcp_sched_from_plan", "fcp_sched_destroy",
     "fcp_sched_workspace_size", "fcp_sched_upload", "fcp_sched_get_info", "fcp_attn_fwd",
-    "fcp_attn_bwd", "fcp_merge",
+    "fcp_attn_bwd", "fcp_merge", "fcp_plan_piece_stats", "fcp_piece_layout", "fcp_kv_gather_piece",
+    "fcp_kv_scatter_add_piece", "fcp_sched_from_plan_piece",
 ]
 
 STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC, STRATEGY_PER_SEQ = 0, 1, 2, 3
+# key sets of a rank (include/fcp.h section 2b): the whole prefix, or its local / prefix split
+PIECE_FULL, PIECE_LOCAL, PIECE_PREFIX = 0, 1, 2
+DQ_KEEP, DQ_NO_OUTPUT = 1, 2
 
 
 class FcpError(RuntimeError):
@@ -67,14 +71,16 @@ class _GatherCounts(C.Structure):
 class _SchedInfo(C.Structure):
     _fields_ = [("n_fwd_items", C.c_int32), ("n_bwd_items", C.c_int32),
                 ("fwd_kv_tiles", C.c_int64), ("bwd_tile_pairs", C.c_int64),
-                ("useful_pairs", C.c_uint64), ("n_q", C.c_int64), ("n_kv", C.c_int64)]
+                ("useful_pairs", C.c_uint64), ("n_q", C.c_int64), ("n_kv", C.c_int64),
+                ("n_q_pad", C.c_int64)]
 
 
 class _AttnArgs(C.Structure):
     _fields_ = [("sched", C.c_void_p), ("workspace", C.c_void_p), ("q", C.c_void_p),
                 ("k", C.c_void_p), ("v", C.c_void_p), ("o", C.c_void_p), ("lse", C.c_void_p),
                 ("scale", C.c_float), ("dkv_dtype", C.c_int32), ("stream", C.c_void_p),
-                ("ev_start", C.c_void_p), ("ev_stop", C.c_void_p)]
+                ("ev_start", C.c_void_p), ("ev_stop", C.c_void_p), ("dq_accum", C.c_void_p),
+                ("dq_flags", C.c_int32)]
 
 
 _LIB = None
@@ -100,17 +106,23 @@ def _lib():
         lib.fcp_plan_perdoc.argtypes = [C.c_void_p, _I32P, C.c_int32, _I32P]
         lib.fcp_plan_stats.argtypes = [C.c_void_p, C.POINTER(_Stats)]
         lib.fcp_plan_rank_stats.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_RankStats)]
+        lib.fcp_plan_piece_stats.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(_RankStats)]
         lib.fcp_rank_layout.argtypes = [C.c_void_p, C.c_int32, C.POINTER(_Layout)]
-        lib.fcp_kv_gather.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
-                                      C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
-                                      C.POINTER(_GatherCounts)]
-        lib.fcp_kv_scatter_add.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32,
-                                           C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
-                                           C.c_void_p, C.POINTER(_GatherCounts)]
+        lib.fcp_piece_layout.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.POINTER(_Layout)]
+        gather = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.c_void_p,
+                  C.POINTER(_GatherCounts)]
+        lib.fcp_kv_gather.argtypes = [C.c_void_p, C.c_int32] + gather
+        lib.fcp_kv_gather_piece.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + gather
+        scatter = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
+                   C.c_void_p, C.POINTER(_GatherCounts)]
+        lib.fcp_kv_scatter_add.argtypes = [C.c_void_p, C.c_int32] + scatter
+        lib.fcp_kv_scatter_add_piece.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + scatter
         lib.fcp_sched_create.argtypes = [_I32P, _I32P, _I32P, C.c_int32, _I32P, C.c_int32,
                                          C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
         lib.fcp_sched_from_plan.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
                                             C.POINTER(C.c_void_p)]
+        lib.fcp_sched_from_plan_piece.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32,
+                                                  C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
         lib.fcp_sched_workspace_size.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         lib.fcp_sched_upload.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.fcp_sched_get_info.argtypes = [C.c_void_p, C.POINTER(_SchedInfo)]
@@ -202,41 +214,42 @@ class Plan:
         _check(_lib().fcp_plan_stats(self._h, C.byref(s)), "fcp_plan_stats")
         return _struct_dict(s)
 
-    def rank_stats(self, rank):
+    def rank_stats(self, rank, piece=PIECE_FULL):
         s = _RankStats()
-        _check(_lib().fcp_plan_rank_stats(self._h, rank, C.byref(s)), "fcp_plan_rank_stats")
+        _check(_lib().fcp_plan_piece_stats(self._h, rank, piece, C.byref(s)), "fcp_plan_piece_stats")
         return _struct_dict(s)
 
-    def rank_layout(self, rank):
+    def rank_layout(self, rank, piece=PIECE_FULL):
         """dict of int32 numpy arrays (see fcp_layout in include/fcp.h)."""
-        rs = self.rank_stats(rank)
+        rs = self.rank_stats(rank, piece)
         ns, ng = rs["n_shards"], rs["n_segs"]
         sizes = {"cu_seqlens_q": ns + 1, "q_pos_off": ns, "shard_seg": ns, "cu_seqlens_k": ng + 1,
                  "kv_src_start": ng, "kv_len": ng, "q_token_index": rs["n_q"],
                  "kv_token_index": rs["n_kv"]}
         arrs = {k: np.zeros(max(1, v), dtype=np.int32) for k, v in sizes.items()}
         lay = _Layout(**{k: _p(a) for k, a in arrs.items()})
-        _check(_lib().fcp_rank_layout(self._h, rank, C.byref(lay)), "fcp_rank_layout")
+        _check(_lib().fcp_piece_layout(self._h, rank, piece, C.byref(lay)), "fcp_piece_layout")
         return {k: arrs[k][:sizes[k]] for k in sizes}
 
-    def kv_gather(self, rank, K, V, k_out=None, v_out=None, stream=None):
-        """Device gather of the rank's KV prefixes.  K, V: torch bf16 [C,Hkv,D] on the GPU.
-        Returns (k_out, v_out, counts)."""
+    def kv_gather(self, rank, K, V, k_out=None, v_out=None, stream=None, piece=PIECE_FULL):
+        """Device gather of the rank's KV prefixes (or of one piece of their local / prefix
+        split).  K, V: torch bf16 [C,Hkv,D] on the GPU.  Returns (k_out, v_out, counts)."""
         import torch
         assert K.is_cuda and V.is_cuda and K.is_contiguous() and V.is_contiguous()
         Hkv, D = K.shape[1], K.shape[2]
-        n_kv = self.rank_stats(rank)["n_kv"]
+        n_kv = self.rank_stats(rank, piece)["n_kv"]
         if k_out is None:
             k_out = torch.empty((n_kv, Hkv, D), dtype=K.dtype, device=K.device)
         if v_out is None:
             v_out = torch.empty((n_kv, Hkv, D), dtype=V.dtype, device=V.device)
         cnt = _GatherCounts()
-        _check(_lib().fcp_kv_gather(self._h, rank, K.data_ptr(), V.data_ptr(), k_out.data_ptr(),
-                                    v_out.data_ptr(), Hkv, D * K.element_size() // 2,
-                                    _stream_ptr(stream), C.byref(cnt)), "fcp_kv_gather")
+        _check(_lib().fcp_kv_gather_piece(self._h, rank, piece, K.data_ptr(), V.data_ptr(),
+                                          k_out.data_ptr(), v_out.data_ptr(), Hkv,
+                                          D * K.element_size() // 2, _stream_ptr(stream),
+                                          C.byref(cnt)), "fcp_kv_gather_piece")
         return k_out, v_out, _struct_dict(cnt)
 
-    def kv_scatter_add(self, rank, dk_r, dv_r, dK, dV, stream=None):
+    def kv_scatter_add(self, rank, dk_r, dv_r, dK, dV, stream=None, piece=PIECE_FULL):
         """dK, dV (fp32 [C,Hkv,D]) += the rank's dk_r, dv_r (bf16 or fp32 [n_kv,Hkv,D], layout of
         the gathered KV).  Returns the counts dict (bytes a ReduceScatter would move)."""
         import torch
@@ -245,18 +258,19 @@ class Plan:
         assert dK.dtype == torch.float32 and dV.dtype == torch.float32
         assert dk_r.dtype == dv_r.dtype and dk_r.dtype in (torch.bfloat16, torch.float32)
         Hkv, D = dK.shape[1], dK.shape[2]
-        assert dk_r.shape[0] == self.rank_stats(rank)["n_kv"] and dk_r.shape[1:] == dK.shape[1:]
+        assert dk_r.shape[0] == self.rank_stats(rank, piece)["n_kv"] and dk_r.shape[1:] == dK.shape[1:]
         cnt = _GatherCounts()
-        _check(_lib().fcp_kv_scatter_add(self._h, rank, dk_r.data_ptr(), dv_r.data_ptr(),
-                                         0 if dk_r.dtype == torch.bfloat16 else 1, dK.data_ptr(),
-                                         dV.data_ptr(), Hkv, D, _stream_ptr(stream), C.byref(cnt)),
-               "fcp_kv_scatter_add")
+        _check(_lib().fcp_kv_scatter_add_piece(self._h, rank, piece, dk_r.data_ptr(), dv_r.data_ptr(),
+                                               0 if dk_r.dtype == torch.bfloat16 else 1,
+                                               dK.data_ptr(), dV.data_ptr(), Hkv, D,
+                                               _stream_ptr(stream), C.byref(cnt)),
+               "fcp_kv_scatter_add_piece")
         return _struct_dict(cnt)
 
-    def sched(self, rank, n_q_heads, n_kv_heads, head_dim):
+    def sched(self, rank, n_q_heads, n_kv_heads, head_dim, piece=PIECE_FULL):
         h = C.c_void_p()
-        _check(_lib().fcp_sched_from_plan(self._h, rank, n_q_heads, n_kv_heads, head_dim,
-                                          C.byref(h)), "fcp_sched_from_plan")
+        _check(_lib().fcp_sched_from_plan_piece(self._h, rank, piece, n_q_heads, n_kv_heads,
+                                                head_dim, C.byref(h)), "fcp_sched_from_plan_piece")
         return Sched(h, n_q_heads, n_kv_heads, head_dim)
 
 
@@ -300,13 +314,21 @@ class Sched:
                "fcp_sched_upload")
         return self
 
-    def _args(self, q, k, v, o, lse, scale, stream, events=None, dkv_f32=False):
+    def _args(self, q, k, v, o, lse, scale, stream, events=None, dkv_f32=False, dq_accum=None,
+              dq_flags=0):
         if self.workspace is None:
             self.upload(q.device)
         ev0, ev1 = (None, None) if events is None else (_event_ptr(e) for e in events)
         return _AttnArgs(self._h, self.workspace.data_ptr(), q.data_ptr(), k.data_ptr(),
                          v.data_ptr(), o.data_ptr(), lse.data_ptr(), float(scale),
-                         1 if dkv_f32 else 0, _stream_ptr(stream), ev0, ev1)
+                         1 if dkv_f32 else 0, _stream_ptr(stream), ev0, ev1,
+                         None if dq_accum is None else dq_accum.data_ptr(), dq_flags)
+
+    def dq_accumulator(self, device="cuda"):
+        """fp32 [Hq, n_q_pad, D] buffer for attn_bwd(dq_accum=...) over several KV pieces."""
+        import torch
+        return torch.empty((self.Hq, self.info()["n_q_pad"], self.D), dtype=torch.float32,
+                           device=device)
 
     def attn_fwd(self, q, k, v, scale, o=None, lse=None, stream=None, events=None):
         """q [n_q,Hq,D], k,v [n_kv,Hkv,D] torch bf16 on the GPU -> (o bf16, lse f32 [Hq,n_q]).
@@ -323,22 +345,29 @@ class Sched:
         return o, lse
 
     def attn_bwd(self, q, k, v, o, lse, do, scale, dq=None, dk=None, dv=None, stream=None,
-                 events=None, dkv_dtype=None):
-        """-> (dq bf16, dk, dv); dk, dv are bf16 unless dkv_dtype (or the given buffers) is f32."""
+                 events=None, dkv_dtype=None, dq_accum=None, dq_flags=0):
+        """-> (dq bf16, dk, dv); dk, dv are bf16 unless dkv_dtype (or the given buffers) is f32.
+        dq_accum / dq_flags (DQ_KEEP, DQ_NO_OUTPUT): dq accumulation over KV pieces, see
+        fcp_attn_args in include/fcp.h; with DQ_NO_OUTPUT the returned dq is None."""
         import torch
         for t in (q, k, v, o, do):
             assert t.is_cuda and t.is_contiguous() and t.dtype == torch.bfloat16
         if dkv_dtype is None:
             dkv_dtype = dk.dtype if dk is not None else torch.bfloat16
         assert dkv_dtype in (torch.bfloat16, torch.float32)
-        dq = torch.empty_like(q) if dq is None else dq
+        assert dq_accum is None or (dq_accum.is_cuda and dq_accum.dtype == torch.float32 and
+                                    dq_accum.numel() == self.Hq * self.info()["n_q_pad"] * self.D)
+        no_out = dq_accum is not None and (dq_flags & DQ_NO_OUTPUT)
+        if not no_out:
+            dq = torch.empty_like(q) if dq is None else dq
         dk = torch.empty_like(k, dtype=dkv_dtype) if dk is None else dk
         dv = torch.empty_like(v, dtype=dkv_dtype) if dv is None else dv
         assert dk.dtype == dkv_dtype and dv.dtype == dkv_dtype
-        a = self._args(q, k, v, o, lse, scale, stream, events, dkv_dtype == torch.float32)
-        _check(_lib().fcp_attn_bwd(C.byref(a), do.data_ptr(), dq.data_ptr(), dk.data_ptr(),
-                                   dv.data_ptr()), "fcp_attn_bwd")
-        return dq, dk, dv
+        a = self._args(q, k, v, o, lse, scale, stream, events, dkv_dtype == torch.float32,
+                       dq_accum, dq_flags)
+        _check(_lib().fcp_attn_bwd(C.byref(a), do.data_ptr(), None if no_out else dq.data_ptr(),
+                                   dk.data_ptr(), dv.data_ptr()), "fcp_attn_bwd")
+        return (None if no_out else dq), dk, dv
 
 
 def merge(o_a, lse_a, o_b, lse_b, o_out=None, lse_out=None, stream=None):

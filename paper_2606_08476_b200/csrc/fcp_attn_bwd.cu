@@ -66,7 +66,8 @@ fcp_bwd_prep(const __nv_bfloat16* __restrict__ o, const __nv_bfloat16* __restric
              int Hq) {
   const int tile = blockIdx.x, head = blockIdx.y;
   // zero this (q tile, head) block of the fp32 dQ accumulator: saves a separate memset pass
-  {
+  // (dq_acc == nullptr: the accumulator holds an earlier KV piece's partial, FCP_DQ_KEEP)
+  if (dq_acc != nullptr) {
     float4* z = dq_acc + ((int64_t)head * n_q_pad + (int64_t)tile * FCP_BQ) * (D / 4);
     for (int i = threadIdx.x; i < FCP_BQ * D / 4; i += blockDim.x) z[i] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
@@ -628,13 +629,18 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
   char* ws = static_cast<char*>(a->workspace);
   const int32_t* tile_meta = reinterpret_cast<const int32_t*>(ws + s->off_shard_meta);
   float2* lsed = reinterpret_cast<float2*>(ws + s->off_lsed);
-  float* dq_acc = reinterpret_cast<float*>(ws + s->off_dq);
+  // dQ accumulates in fp32 across the KV tiles — and, with a caller-owned accumulator, across
+  // the KV pieces of a local / prefix split (fcp.h section 2b)
+  float* dq_acc = a->dq_accum ? a->dq_accum : reinterpret_cast<float*>(ws + s->off_dq);
+  const bool keep = a->dq_accum && (a->dq_flags & FCP_DQ_KEEP);
+  const bool convert = !(a->dq_accum && (a->dq_flags & FCP_DQ_NO_OUTPUT));
   const int n_pad_tiles = (int)(s->n_q_pad / FCP_BQ);
 
   if (n_pad_tiles > 0) {
     fcp_bwd_prep<D><<<dim3(n_pad_tiles, s->Hq), 256, 0, st>>>(
         static_cast<const __nv_bfloat16*>(a->o), static_cast<const __nv_bfloat16*>(dO), a->lse,
-        tile_meta, lsed, reinterpret_cast<float4*>(dq_acc), s->n_q, s->n_q_pad, s->Hq);
+        tile_meta, lsed, keep ? nullptr : reinterpret_cast<float4*>(dq_acc), s->n_q, s->n_q_pad,
+        s->Hq);
     if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
   }
   const int n_items = (int)s->bwd.size();
@@ -661,7 +667,7 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
     if (a->ev_stop && cudaEventRecord((cudaEvent_t)a->ev_stop, st) != cudaSuccess)
       return FCP_CUDA;
   }
-  if (n_pad_tiles > 0) {
+  if (n_pad_tiles > 0 && convert) {
     fcp_bwd_dq_convert<D><<<dim3(n_pad_tiles, s->Hq), 256, 0, st>>>(
         dq_acc, tile_meta, static_cast<__nv_bfloat16*>(dq), s->n_q_pad, s->Hq, a->scale);
     if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;
@@ -672,9 +678,11 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
 }  // namespace
 
 extern "C" int fcp_attn_bwd(const fcp_attn_args* a, const void* dO, void* dq, void* dk, void* dv) {
-  if (!a || !a->sched || !a->workspace || !a->q || !a->k || !a->v || !a->o || !a->lse || !dO ||
-      !dq || !dk || !dv)
-    return FCP_INVALID_ARG;
+  if (!a || !a->sched || !a->workspace || !a->q || !a->o || !a->lse || !dO) return FCP_INVALID_ARG;
+  // k, v, dk, dv may be NULL when the schedule has no key at all (n_kv == 0)
+  if (a->sched->n_kv > 0 && (!a->k || !a->v || !dk || !dv)) return FCP_INVALID_ARG;
+  if (!dq && !(a->dq_accum && (a->dq_flags & FCP_DQ_NO_OUTPUT))) return FCP_INVALID_ARG;
+  if (a->dq_accum && (reinterpret_cast<uintptr_t>(a->dq_accum) & 15)) return FCP_MISALIGNED;
   const fcp_sched* s = a->sched;
   if (a->dkv_dtype != FCP_DTYPE_BF16 && a->dkv_dtype != FCP_DTYPE_F32) return FCP_UNSUPPORTED;
   for (const void* p : {a->q, a->k, a->v, (const void*)a->o, (const void*)a->workspace, dO,

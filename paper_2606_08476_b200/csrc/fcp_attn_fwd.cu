@@ -522,9 +522,13 @@ template <int D, int NQ>
 int launch_fwd(const fcp_attn_args* a, const fcp_sched* s) {
   using Cfg = FwdCfg<D, NQ>;
   CUtensorMap mq, mk, mv;
+  // an empty KV buffer (n_kv == 0: a PREFIX piece of shards that all start their document) has
+  // no tile to load; its maps only need a valid base
+  const void* kb = s->n_kv > 0 ? a->k : a->q;
+  const void* vb = s->n_kv > 0 ? a->v : a->q;
   if (!make_tmap_rows(&mq, a->q, D, s->Hq, s->n_q, 128) ||
-      !make_tmap_rows(&mk, a->k, D, s->Hkv, s->n_kv, 128) ||
-      !make_tmap_rows(&mv, a->v, D, s->Hkv, s->n_kv, 128))
+      !make_tmap_rows(&mk, kb, D, s->Hkv, s->n_kv, 128) ||
+      !make_tmap_rows(&mv, vb, D, s->Hkv, s->n_kv, 128))
     return FCP_CUDA;
   auto kern = fcp_attn_fwd_kernel<D, NQ>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes) !=
@@ -547,9 +551,9 @@ int launch_fwd(const fcp_attn_args* a, const fcp_sched* s) {
 }  // namespace
 
 extern "C" int fcp_attn_fwd(const fcp_attn_args* a) {
-  if (!a || !a->sched || !a->workspace || !a->q || !a->k || !a->v || !a->o || !a->lse)
-    return FCP_INVALID_ARG;
+  if (!a || !a->sched || !a->workspace || !a->q || !a->o || !a->lse) return FCP_INVALID_ARG;
   const fcp_sched* s = a->sched;
+  if (s->n_kv > 0 && (!a->k || !a->v)) return FCP_INVALID_ARG;   // k, v may be NULL when n_kv == 0
   for (const void* p : {a->q, a->k, a->v, (const void*)a->o, (const void*)a->workspace})
     if (reinterpret_cast<uintptr_t>(p) & 15) return FCP_MISALIGNED;
   if (s->fwd.empty()) return FCP_OK;

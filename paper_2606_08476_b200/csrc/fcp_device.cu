@@ -221,13 +221,23 @@ fcp_merge_kernel(const void* __restrict__ o_a, const float* __restrict__ lse_a,
 }
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15) == 0; }
+bool valid_piece(int32_t piece) {
+  return piece == FCP_PIECE_FULL || piece == FCP_PIECE_LOCAL || piece == FCP_PIECE_PREFIX;
+}
 
 }  // namespace
 
 extern "C" int fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, const void* V,
                              void* k_out, void* v_out, int32_t n_kv_heads, int32_t head_dim,
                              void* stream, fcp_gather_counts* counts) {
-  if (!plan || rank < 0 || rank >= plan->n_ranks || !K || !V || !k_out || !v_out ||
+  return fcp_kv_gather_piece(plan, rank, FCP_PIECE_FULL, K, V, k_out, v_out, n_kv_heads, head_dim,
+                             stream, counts);
+}
+
+extern "C" int fcp_kv_gather_piece(const fcp_plan* plan, int32_t rank, int32_t piece, const void* K,
+                                   const void* V, void* k_out, void* v_out, int32_t n_kv_heads,
+                                   int32_t head_dim, void* stream, fcp_gather_counts* counts) {
+  if (!plan || rank < 0 || rank >= plan->n_ranks || !valid_piece(piece) || !K || !V ||
       n_kv_heads < 1 || head_dim < 1)
     return FCP_INVALID_ARG;
   const int64_t row_bytes = (int64_t)n_kv_heads * head_dim * 2;
@@ -235,10 +245,12 @@ extern "C" int fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, 
   if (!aligned16(K) || !aligned16(V) || !aligned16(k_out) || !aligned16(v_out))
     return FCP_MISALIGNED;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v);
+  fcp_build_rank_view(*plan, rank, v, piece);
+  if (v.n_kv > 0 && (!k_out || !v_out)) return FCP_INVALID_ARG;   // an empty piece needs no buffer
   // merge ranges that are contiguous in the source (neighbouring documents held whole)
   std::vector<int64_t> src, len;
   for (size_t g = 0; g < v.kv_len.size(); ++g) {
+    if (v.kv_len[g] == 0) continue;
     if (!src.empty() && src.back() + len.back() == v.kv_src_start[g]) {
       len.back() += v.kv_len[g];
     } else {
@@ -295,7 +307,15 @@ extern "C" int fcp_kv_scatter_add(const fcp_plan* plan, int32_t rank, const void
                                   const void* dv_r, int32_t src_dtype, float* dK, float* dV,
                                   int32_t n_kv_heads, int32_t head_dim, void* stream,
                                   fcp_gather_counts* counts) {
-  if (!plan || rank < 0 || rank >= plan->n_ranks || !dk_r || !dv_r || !dK || !dV ||
+  return fcp_kv_scatter_add_piece(plan, rank, FCP_PIECE_FULL, dk_r, dv_r, src_dtype, dK, dV,
+                                  n_kv_heads, head_dim, stream, counts);
+}
+
+extern "C" int fcp_kv_scatter_add_piece(const fcp_plan* plan, int32_t rank, int32_t piece,
+                                        const void* dk_r, const void* dv_r, int32_t src_dtype,
+                                        float* dK, float* dV, int32_t n_kv_heads, int32_t head_dim,
+                                        void* stream, fcp_gather_counts* counts) {
+  if (!plan || rank < 0 || rank >= plan->n_ranks || !valid_piece(piece) || !dK || !dV ||
       n_kv_heads < 1 || head_dim < 1)
     return FCP_INVALID_ARG;
   if (src_dtype != FCP_DTYPE_BF16 && src_dtype != FCP_DTYPE_F32) return FCP_UNSUPPORTED;
@@ -303,9 +323,11 @@ extern "C" int fcp_kv_scatter_add(const fcp_plan* plan, int32_t rank, const void
   if (row_elems % 8 != 0) return FCP_UNSUPPORTED;
   if (!aligned16(dk_r) || !aligned16(dv_r) || !aligned16(dK) || !aligned16(dV)) return FCP_MISALIGNED;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v);
+  fcp_build_rank_view(*plan, rank, v, piece);
+  if (v.n_kv > 0 && (!dk_r || !dv_r)) return FCP_INVALID_ARG;     // an empty piece needs no buffer
   std::vector<int64_t> tok, len;                  // merged destination ranges (global tokens)
   for (size_t g = 0; g < v.kv_len.size(); ++g) {
+    if (v.kv_len[g] == 0) continue;
     if (!tok.empty() && tok.back() + len.back() == v.kv_src_start[g]) {
       len.back() += v.kv_len[g];
     } else {
@@ -327,15 +349,21 @@ extern "C" int fcp_kv_scatter_add(const fcp_plan* plan, int32_t rank, const void
   if (cudaGetDevice(&dev) != cudaSuccess) return FCP_CUDA;
   cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
   int64_t src_row = 0;
-  for (size_t base = 0; base < tok.size(); base += kMaxRanges) {
+  for (size_t base = 0; base < tok.size();) {
+    // one launch = a run of buffer-contiguous ranges with pairwise distinct destination tokens.
+    // Ranges are in (document, start) order, so a range can only overlap the one before it (a
+    // PREFIX piece repeats a prefix when the rank holds two shards of one document): such a
+    // range opens the next launch, ordered after this one on the stream.
     GatherRanges rg;
     std::memset(&rg, 0, sizeof(rg));
-    rg.n = (int32_t)std::min<size_t>(kMaxRanges, tok.size() - base);
-    int64_t c = 0;
-    for (int i = 0; i < rg.n; ++i) {
-      rg.dst0[i] = c;                             // position in the rank buffer
-      rg.src0[i] = tok[base + i] * upr;           // position in the global accumulator
-      c += len[base + i] * upr;
+    int64_t c = 0, run_end = -1;
+    while (base < tok.size() && rg.n < kMaxRanges && tok[base] >= run_end) {
+      rg.dst0[rg.n] = c;                          // position in the rank buffer
+      rg.src0[rg.n] = tok[base] * upr;            // position in the global accumulator
+      c += len[base] * upr;
+      run_end = std::max(run_end, tok[base] + len[base]);
+      ++rg.n;
+      ++base;
     }
     rg.dst0[rg.n] = c;
     const int64_t spans = 2 * ((c + kScatterThreads * kScatterUnroll - 1) / (kScatterThreads * kScatterUnroll));

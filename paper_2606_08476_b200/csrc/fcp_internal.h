@@ -23,7 +23,10 @@ struct RankView {
   int64_t n_q = 0, n_kv = 0, remote = 0, nonlast = 0;
   uint64_t load = 0;
 };
-void fcp_build_rank_view(const fcp_plan& p, int32_t rank, RankView& v);
+// piece: FCP_PIECE_FULL (one segment per document prefix) or the local / prefix split (one
+// segment per shard, fcp.h section 2b)
+void fcp_build_rank_view(const fcp_plan& p, int32_t rank, RankView& v,
+                         int32_t piece = FCP_PIECE_FULL);
 
 inline uint64_t fcp_W(uint64_t p, uint64_t s) { return (2 * p + s + 1) * s / 2; }
 

@@ -240,7 +240,7 @@ extern "C" int fcp_plan_perdoc(const fcp_plan* plan, int32_t* doc_ids, int32_t c
   return cnt > cap ? FCP_BUFFER_TOO_SMALL : FCP_OK;
 }
 
-void fcp_build_rank_view(const fcp_plan& p, int32_t rank, RankView& v) {
+void fcp_build_rank_view(const fcp_plan& p, int32_t rank, RankView& v, int32_t piece) {
   const int n = (int)p.d.size();
   std::vector<int32_t> E(n, 0), seg_of(n, -1);
   const int32_t b = p.rank_begin[rank], e = p.rank_begin[rank + 1];
@@ -270,12 +270,42 @@ void fcp_build_rank_view(const fcp_plan& p, int32_t rank, RankView& v) {
   }
   v.n_q = v.cu_q.back();
   v.remote = v.n_kv - own_in_prefix;
+  if (piece == FCP_PIECE_FULL) return;
+  // Local / prefix split (fcp.h section 2b): one KV segment per shard.  LOCAL = the shard's own
+  // tokens [p, p+s), causal from its first key; PREFIX = the tokens [0, p) before it, all
+  // visible.  The distinct remote tokens of PREFIX are those of the unsplit gather.
+  v.cu_k.assign(1, 0);
+  v.kv_src_start.clear();
+  v.kv_len.clear();
+  v.seg_doc.clear();
+  for (int32_t i = b; i < e; ++i) {
+    const fcp_shard& s = p.shards[i];
+    const bool local = piece == FCP_PIECE_LOCAL;
+    v.q_pos_off[i - b] = local ? 0 : s.start;
+    v.shard_seg[i - b] = i - b;
+    v.kv_src_start.push_back((int32_t)(p.off[s.doc] + (local ? s.start : 0)));
+    v.kv_len.push_back(local ? s.len : s.start);
+    v.seg_doc.push_back(s.doc);
+    v.cu_k.push_back(v.cu_k.back() + v.kv_len.back());
+  }
+  v.n_kv = v.cu_k.back();
+  if (piece == FCP_PIECE_LOCAL) v.remote = 0;
+}
+
+static bool valid_piece(int32_t piece) {
+  return piece == FCP_PIECE_FULL || piece == FCP_PIECE_LOCAL || piece == FCP_PIECE_PREFIX;
 }
 
 extern "C" int fcp_plan_rank_stats(const fcp_plan* plan, int32_t rank, fcp_rank_stats* out) {
-  if (!plan || !out || rank < 0 || rank >= plan->n_ranks) return FCP_INVALID_ARG;
+  return fcp_plan_piece_stats(plan, rank, FCP_PIECE_FULL, out);
+}
+
+extern "C" int fcp_plan_piece_stats(const fcp_plan* plan, int32_t rank, int32_t piece,
+                                    fcp_rank_stats* out) {
+  if (!plan || !out || rank < 0 || rank >= plan->n_ranks || !valid_piece(piece))
+    return FCP_INVALID_ARG;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v);
+  fcp_build_rank_view(*plan, rank, v, piece);
   out->n_shards = (int32_t)v.q_pos_off.size();
   out->n_segs = (int32_t)v.kv_len.size();
   out->n_q = v.n_q;
@@ -317,9 +347,15 @@ extern "C" int fcp_plan_stats(const fcp_plan* plan, fcp_stats* out) {
 }
 
 extern "C" int fcp_rank_layout(const fcp_plan* plan, int32_t rank, fcp_layout* out) {
-  if (!plan || !out || rank < 0 || rank >= plan->n_ranks) return FCP_INVALID_ARG;
+  return fcp_piece_layout(plan, rank, FCP_PIECE_FULL, out);
+}
+
+extern "C" int fcp_piece_layout(const fcp_plan* plan, int32_t rank, int32_t piece,
+                                fcp_layout* out) {
+  if (!plan || !out || rank < 0 || rank >= plan->n_ranks || !valid_piece(piece))
+    return FCP_INVALID_ARG;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v);
+  fcp_build_rank_view(*plan, rank, v, piece);
   auto put = [](int32_t* dst, const std::vector<int32_t>& src) {
     if (dst && !src.empty()) std::memcpy(dst, src.data(), sizeof(int32_t) * src.size());
   };

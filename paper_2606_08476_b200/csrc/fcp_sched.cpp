@@ -198,9 +198,17 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
 
 extern "C" int fcp_sched_from_plan(const fcp_plan* plan, int32_t rank, int32_t n_q_heads,
                                    int32_t n_kv_heads, int32_t head_dim, fcp_sched** out) {
-  if (!plan || !out || rank < 0 || rank >= plan->n_ranks) return FCP_INVALID_ARG;
+  return fcp_sched_from_plan_piece(plan, rank, FCP_PIECE_FULL, n_q_heads, n_kv_heads, head_dim, out);
+}
+
+extern "C" int fcp_sched_from_plan_piece(const fcp_plan* plan, int32_t rank, int32_t piece,
+                                         int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                                         fcp_sched** out) {
+  if (!plan || !out || rank < 0 || rank >= plan->n_ranks ||
+      (piece != FCP_PIECE_FULL && piece != FCP_PIECE_LOCAL && piece != FCP_PIECE_PREFIX))
+    return FCP_INVALID_ARG;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v);
+  fcp_build_rank_view(*plan, rank, v, piece);
   return fcp_sched_create(v.cu_q.data(), v.q_pos_off.data(), v.shard_seg.data(),
                           (int32_t)v.q_pos_off.size(), v.cu_k.data(), (int32_t)v.kv_len.size(),
                           n_q_heads, n_kv_heads, head_dim, out);
@@ -223,5 +231,6 @@ extern "C" int fcp_sched_get_info(const fcp_sched* sched, fcp_sched_info* out) {
   out->useful_pairs = sched->useful_pairs;
   out->n_q = sched->n_q;
   out->n_kv = sched->n_kv;
+  out->n_q_pad = sched->n_q_pad;
   return FCP_OK;
 }

@@ -74,6 +74,39 @@ def run_rank_gpu(fcp, plan, rank, Q, K, V, dO, scale, do_bwd=True, dkv_f32=False
     return out
 
 
+def run_rank_split_gpu(fcp, plan, rank, Q, K, V, dO, scale, dK, dV):
+    """The same path with the rank's keys split into the LOCAL and the PREFIX piece (include/fcp.h
+    section 2b): two forwards + fcp_merge, two backwards that share one fp32 dq accumulator,
+    dk / dv of both pieces scatter-added into the global fp32 dK, dV."""
+    import torch
+    Hq, Hkv, D = Q.shape[1], K.shape[1], Q.shape[2]
+    lay = plan.rank_layout(rank)
+    qi = torch.from_numpy(lay["q_token_index"].astype(np.int64)).to(Q.device)
+    q, do = Q[qi].contiguous(), dO[qi].contiguous()
+    part = {}
+    for piece in (fcp.PIECE_LOCAL, fcp.PIECE_PREFIX):
+        k, v, counts = plan.kv_gather(rank, K, V, piece=piece)
+        sched = plan.sched(rank, Hq, Hkv, D, piece).upload(Q.device)
+        o, lse = sched.attn_fwd(q, k, v, scale)
+        part[piece] = dict(k=k, v=v, counts=counts, sched=sched, o=o, lse=lse)
+    loc, pre = part[fcp.PIECE_LOCAL], part[fcp.PIECE_PREFIX]
+    o, lse = fcp.merge(loc["o"], loc["lse"], pre["o"], pre["lse"])
+    acc = loc["sched"].dq_accumulator(Q.device)
+    acc.fill_(float("nan"))                       # the first piece must zero it itself
+    dq0, loc["dk"], loc["dv"] = loc["sched"].attn_bwd(
+        q, loc["k"], loc["v"], o, lse, do, scale, dkv_dtype=torch.float32, dq_accum=acc,
+        dq_flags=fcp.DQ_NO_OUTPUT)
+    assert dq0 is None
+    dq, pre["dk"], pre["dv"] = pre["sched"].attn_bwd(
+        q, pre["k"], pre["v"], o, lse, do, scale, dkv_dtype=torch.float32, dq_accum=acc,
+        dq_flags=fcp.DQ_KEEP)
+    for piece in (fcp.PIECE_LOCAL, fcp.PIECE_PREFIX):
+        part[piece]["scatter"] = plan.kv_scatter_add(rank, part[piece]["dk"], part[piece]["dv"],
+                                                     dK, dV, piece=piece)
+    torch.cuda.synchronize()
+    return {"o": o, "lse": lse, "dq": dq, "layout": lay, "local": loc, "prefix": pre}
+
+
 def run_rank_oracle(d, N, rank, Q, K, V, dO, scale, r_ppm=1_050_000, strategy=0, do_bwd=True):
     """Same rank through oracle/ (fp64).  Q,K,V,dO are numpy fp64 arrays in global order."""
     pl = OP.plan(d, N, r_ppm, strategy)

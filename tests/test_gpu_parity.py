@@ -311,6 +311,57 @@ def test_kv_scatter_add_matches_oracle(fcp, torch, name, strategy, src):
     assert total_remote == plan.stats()["sum_remote_tokens"]
 
 
+SPLIT_CASES = [
+    # d, N, Hq, Hkv, D, strategy
+    ([900, 260, 250, 126], 4, 4, 2, 128, 0),       # hybrid: whole documents + one sharded
+    ([700, 500, 400, 192], 2, 4, 2, 64, 1),        # all Per-Doc: two shards per document and rank,
+                                                   # the PREFIX buffer repeats a prefix
+    ([129, 127, 65, 63], 1, 4, 1, 128, 2),         # N=1: every prefix is empty (n_kv = 0)
+    ([900, 50, 700, 270, 128], 4, 4, 2, 128, 3),   # Per-Seq chunks
+    ([2048], 4, 8, 2, 128, 0),                     # one document in 8 chunks
+]
+
+
+@pytest.mark.parametrize("case", SPLIT_CASES, ids=lambda c: "d%d_N%d_D%d_s%d" % (
+    len(c[0]), c[1], c[4], c[5]))
+def test_local_prefix_split_matches_packed_oracle(fcp, torch, case):
+    """per rank, forward over the LOCAL and the PREFIX
+    piece merged by fcp_merge, backward per piece with the merged o / lse, dq accumulated in
+    fp32 across the pieces, dk / dv of the pieces scatter-added into the global fp32 dK / dV —
+    every step a library kernel.  All ranks together must reproduce the packed per-document
+    definition, to the north-star tolerances; the gathered piece buffers and the
+    byte counts are bit-exact against oracle.kvselect."""
+    d, N, Hq, Hkv, D, strategy = case
+    scale = 1.0 / math.sqrt(D)
+    C = sum(d)
+    Q, K, V, dO = fcp_inputs.make_tensors(C, Hq, Hkv, D, 12)
+    f = U.to_f64
+    want_o, want_lse = OA.packed_fwd(f(Q), f(K), f(V), d, scale)
+    want_dq, want_dk, want_dv = OA.packed_bwd(f(Q), f(K), f(V), f(dO), d, scale)
+    plan, opl = fcp.Plan(d, N, 0, strategy), OP.plan(d, N, strategy=strategy)
+    dK = torch.zeros((C, Hkv, D), dtype=torch.float32, device="cuda")
+    dV = torch.zeros_like(dK)
+    o, lse, dq = np.zeros_like(want_o), np.zeros_like(want_lse), np.zeros_like(want_dq)
+    Qd, Kd, Vd, dOd = Q.cuda(), K.cuda(), V.cuda(), dO.cuda()
+    for r in range(N):
+        g = U.run_rank_split_gpu(fcp, plan, r, Qd, Kd, Vd, dOd, scale, dK, dV)
+        qi = g["layout"]["q_token_index"]
+        o[qi], lse[:, qi], dq[qi] = f(g["o"]), f(g["lse"]), f(g["dq"])
+        for key, opiece in (("local", OKV.PIECE_LOCAL), ("prefix", OKV.PIECE_PREFIX)):
+            gi = torch.from_numpy(OKV.piece_gather_index(opl, r, opiece).astype(np.int64))
+            assert torch.equal(g[key]["k"].cpu(), K[gi]) and torch.equal(g[key]["v"].cpu(), V[gi])
+            remote = OKV.piece_remote_tokens(opl, r, opiece)
+            for cnt in (g[key]["counts"], g[key]["scatter"]):
+                assert cnt["total_tokens"] == len(gi) and cnt["remote_tokens"] == remote
+        assert g["local"]["counts"]["remote_bytes"] == 0
+        assert g["prefix"]["counts"]["remote_bytes"] == 2 * OKV.kv_stats(opl).remote[r] * Hkv * D * 2
+    U.check("o", o, want_o)
+    U.check_lse("lse", lse, want_lse)
+    U.check("dq", dq, want_dq)
+    U.check("dk", f(dK), want_dk)
+    U.check("dv", f(dV), want_dv)
+
+
 def test_outputs_do_not_write_out_of_bounds(fcp, torch):
     """Canary rows around every output (o, lse, dq, dk, dv, gathered k/v) on ragged shapes whose
     last tiles are partial: the kernels predicate their stores by q_rows / kv_rows and TMA boxes

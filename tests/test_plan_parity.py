@@ -97,3 +97,42 @@ def test_per_seq_random_and_errors(fcp):
     assert e.value.status == -1
     with pytest.raises(ValueError):
         P.plan([10, 4], 2, strategy=3)
+
+
+def test_piece_layouts_match_oracle(fcp):
+    """Local / prefix split (include/fcp.h section 2b): layouts, token index
+    lists and remote counts bit-exact against oracle/kvselect.piece_*; the two schedules' useful
+    pairs are the two terms of W(p, s) and add up to the unsplit schedule's."""
+    cases = list(random_inputs(21, 40))
+    cases += [(fcp_inputs.doc_lengths(n, 0), fcp_inputs.CONFIGS[n].N, 0, 0) for n in ("tiny", "8b")]
+    for d, N, r_ppm, strategy in cases:
+        want = P.plan(d, N, r_ppm or P.DEFAULT_R_PPM, strategy)
+        got = fcp.Plan(d, N, r_ppm, strategy)
+        for r in range(N):
+            full = got.rank_stats(r)
+            pairs = {}
+            for piece, opiece in ((fcp.PIECE_LOCAL, KV.PIECE_LOCAL), (fcp.PIECE_PREFIX, KV.PIECE_PREFIX)):
+                olay = KV.piece_layout(want, r, opiece)
+                lay = got.rank_layout(r, piece)
+                for key in ("cu_seqlens_q", "q_pos_off", "shard_seg", "cu_seqlens_k", "kv_src_start",
+                            "kv_len"):
+                    assert lay[key].tolist() == getattr(olay, key).tolist(), key
+                assert np.array_equal(lay["q_token_index"], KV.q_token_index(want, r))
+                assert np.array_equal(lay["kv_token_index"], KV.piece_gather_index(want, r, opiece))
+                rs = got.rank_stats(r, piece)
+                assert rs["n_segs"] == rs["n_shards"] == full["n_shards"]
+                assert rs["n_q"] == full["n_q"] and rs["n_kv"] == int(olay.kv_len.sum())
+                assert rs["remote_tokens"] == KV.piece_remote_tokens(want, r, opiece)
+                assert rs["load"] == full["load"]
+                if len(d) <= 16 or r == 0:
+                    pairs[piece] = got.sched(r, 4, 2, 64, piece).info()
+            if pairs:
+                mine = [s for s in want.shards if s.rank == r]
+                assert pairs[fcp.PIECE_LOCAL]["useful_pairs"] == sum(s.len * (s.len + 1) // 2 for s in mine)
+                assert pairs[fcp.PIECE_PREFIX]["useful_pairs"] == sum(s.start * s.len for s in mine)
+                assert pairs[fcp.PIECE_LOCAL]["n_q_pad"] == pairs[fcp.PIECE_PREFIX]["n_q_pad"] \
+                    == got.sched(r, 4, 2, 64).info()["n_q_pad"]
+    with pytest.raises(fcp.FcpError):
+        got.rank_stats(0, 3)
+    with pytest.raises(fcp.FcpError):
+        got.sched(0, 4, 2, 64, piece=7)

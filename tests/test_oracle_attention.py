@@ -289,3 +289,59 @@ def test_local_prefix_split_merges_to_the_packed_result():
                     np.add.at(dv, gi, dv_p)
             for g, w in zip((o, lse, dq, dk, dv), (want_o, want_lse, want_dq, want_dk, want_dv)):
                 np.testing.assert_allclose(g, w, atol=1e-11)
+
+
+def _arbitrary_plans():
+    """hypothesis strategy: ANY exact cover of the documents by shards with ANY rank assignment
+    (not the planner's output, not token-balanced) — SURVEY 8(c1) pin 4."""
+    from hypothesis import strategies as st
+
+    @st.composite
+    def build(draw):
+        n = draw(st.integers(1, 4))
+        d = [draw(st.integers(1, 24)) for _ in range(n)]
+        N = draw(st.integers(1, 4))
+        shards = []
+        for k, dk in enumerate(d):
+            cuts = sorted(set(draw(st.lists(st.integers(1, dk), max_size=4)) + [dk]))
+            a = 0
+            for b in cuts:
+                if b > a:
+                    shards.append(P.Shard(k, a, b - a, draw(st.integers(0, N - 1))))
+                    a = b
+        shards.sort(key=lambda s: (s.rank, s.doc, s.start))
+        merged = []                      # canonical form: contiguous neighbours on a rank merged
+        for s in shards:
+            m = merged[-1] if merged else None
+            if m and (m.rank, m.doc) == (s.rank, s.doc) and m.start + m.len == s.start:
+                merged[-1] = P.Shard(m.doc, m.start, m.len + s.len, m.rank)
+            else:
+                merged.append(s)
+        return P.Plan(tuple(d), N, tuple(merged), (), ())
+    return build()
+
+
+def test_plan_invariance_for_arbitrary_valid_plans():
+    from hypothesis import given, settings, HealthCheck
+
+    @settings(max_examples=40, deadline=None, derandomize=True,
+              suppress_health_check=list(HealthCheck))
+    @given(_arbitrary_plans())
+    def check(pl):
+        rng = np.random.default_rng(len(pl.shards) * 1000 + sum(pl.d))
+        Hq, Hkv, D, scale = 2, 1, 4, 0.45
+        C = sum(pl.d)
+        Q, K, V, dO = rnd(rng, C, Hq, D), rnd(rng, C, Hkv, D), rnd(rng, C, Hkv, D), rnd(rng, C, Hq, D)
+        want_o, want_lse = A.packed_fwd(Q, K, V, list(pl.d), scale)
+        want = (want_o, want_lse) + A.packed_bwd(Q, K, V, dO, list(pl.d), scale)
+        for g, w in zip(run_plan(pl, Q, K, V, dO, scale), want):
+            np.testing.assert_allclose(g, w, atol=1e-11)
+        # and the gather list of every rank is exactly what its rows need
+        for r in range(pl.n_ranks):
+            need = set()
+            off = KV.doc_offsets(pl.d)
+            for s in pl.shards:
+                if s.rank == r:
+                    need.update(range(off[s.doc], off[s.doc] + s.start + s.len))
+            assert sorted(need) == list(KV.gather_index(pl, r))
+    check()

@@ -536,7 +536,10 @@ def run_fcp(args):
         ems = max_over_ranks(t0.elapsed_time(t1))
         e2e = {"value": total_flops / (ems * 1e-3) / 1e12, "unit": "TFLOP/s",
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-               "ms_per_step": ems / args.steps}
+               "ms_per_step": ems / args.steps,
+               # what the step got out of PCIe (it is bound by it; varies from box to box)
+               "h2d_gbs": h2d * args.steps / (ems * 1e-3) / 1e9,
+               "d2h_gbs": d2h * args.steps / (ems * 1e-3) / 1e9}
 
     compare = plan_compare(fcp, w, scale) if (args.plan_compare and rank == 0) else None
     split = split_compare(fcp, w, scale) if (args.split_compare and rank == 0) else None

@@ -1,6 +1,7 @@
 /* fcp.h — C ABI of libfcp: the per-CP-rank hot path of FlashCP (arxiv/paper_2606_08476),
  * B200 / sm_100a.  plan -> rank layout -> sharding-aware KV gather -> document-masked causal
- * attention forward/backward -> partial-result (LSE) merge.
+ * attention forward/backward -> partial-result (LSE) merge; plus the dK/dV scatter-add (the
+ * ReduceScatter stand-in, section 2) and the local / prefix split of a rank's keys (section 2b).
  *
  * Conventions (section 3.1): documents D=[d_0..d_{n-1}] packed in this order into a
  * context of C = sum d_k tokens; CP size N ("ranks"); a shard = (doc, start p, len s, rank) =

@@ -319,6 +319,8 @@ SPLIT_CASES = [
     ([129, 127, 65, 63], 1, 4, 1, 128, 2),         # N=1: every prefix is empty (n_kv = 0)
     ([900, 50, 700, 270, 128], 4, 4, 2, 128, 3),   # Per-Seq chunks
     ([2048], 4, 8, 2, 128, 0),                     # one document in 8 chunks
+    ([1001, 515, 300, 232], 2, 2, 1, 64, 1),       # Per-Doc with remainders: three shards of one
+                                                   # document on a rank, nested prefixes
 ]
 
 

@@ -2,24 +2,30 @@
 //
 // One persistent CTA per SM.  A work item is one 128-row q tile of one shard for a pack of NQ
 // query heads that share a kv head (GQA): the NQ tiles share every K/V tile staged in shared
-// memory.  The pipeline keeps the tensor pipe and the MUFU busy at the same time:
-//   S_t(j+1) = Q_t K_{j+1}^T is issued as soon as the softmax of tile j has LOADED S_t(j) into
-//   registers (P does not alias S: it goes through shared memory), so the softmax warps run
-//   back to back and O_t += P_t(j) V_j only has to keep up.
+// memory.  Per q tile t the chain is   S_t(j) -> softmax -> P_t(j) -> O_t += P_t(j) V_j ->
+// S_t(j+1) = Q_t K_{j+1}^T -> ...   The bf16 P_t is written by the softmax threads over the
+// first 64 TMEM columns of S_t (whose fp32 scores they hold in registers by then) and is the A
+// operand of the PV product straight from TMEM, so that product reads only V from shared memory
+// and no P ever crosses it.  The two tiles' chains alternate: while the tensor pipe works on
+// tile t, the softmax of the other tile has the MUFU to itself (a named-barrier token keeps the
+// two from exponentiating at the same time: two warps per sub-partition in lockstep idle the
+// MUFU during their loads and stores).
 //
-//   warp 0      TMA producer   Q (once per item); K/V tiles through a 3-slot ring in the order
-//                              the MMAs consume them: K0, K1, V0, K2, V1, ...
-//   warp 1      MMA issuer     one elected thread; per KV tile j: S_t(j+1) (SS), then
-//                              O_t += P_t(j) V_j (SS: A = P in swizzled smem, B = V MN-major);
-//                              it probes the next group's barriers before the last MMAs of the
-//                              current group (the tcgen05 queue is ~5 deep)
+//   warp 0      TMA producer   Q (once per item); K/V tiles through a 5-slot ring in the order
+//                              the MMAs consume them: K0, V0, K1, V1, ...
+//   warp 1      MMA issuer     one elected thread; per KV tile j and q tile t: O_t += P_t(j) V_j
+//                              (A = P from TMEM, B = V MN-major), then S_t(j+1) (SS) — program
+//                              order on the in-order tensor pipe is what protects P_t(j) from
+//                              S_t(j+1)
 //   warps 4..   softmax        one warpgroup per q tile, one query row per thread: mask from
 //                              (q_pos0 + row, kv_len), online softmax in the log2 domain that
 //                              exponentiates against the running max of the earlier tiles (no
 //                              max -> exp dependency) and rescales O only when a row grew by
-//                              more than 2^8; bf16 P into shared memory; epilogue o = O / l
+//                              more than 2^8; a quarter of the exponentials of that fast path
+//                              run as a degree-3 polynomial on the FMA pipe (packed fp32x2),
+//                              the rest on the MUFU; epilogue o = O / l
 //
-// TMEM columns: S_t at 128 t, O_t at 128 (NQ + t).
+// TMEM columns: S_t at 128 t (P_t over its first 64), O_t at 128 (NQ + t).
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -48,9 +54,31 @@ using namespace fcp;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 #ifndef FCP_TOKEN_QUARTER
-#define FCP_TOKEN_QUARTER 0
+#define FCP_TOKEN_QUARTER 3
 #endif
 constexpr int kTokenQuarter = FCP_TOKEN_QUARTER;   // quarter of the exponential loop after which the MUFU token moves on
+#ifndef FCP_POLY_MASK
+#define FCP_POLY_MASK 0x55
+#endif
+// Of the 8 groups of 4 scores in a 32-column chunk, the groups whose bit is set here take 2 of
+// their 4 exponentials from the FMA pipe instead of the MUFU (0x55 = a quarter of all ex2)
+constexpr unsigned kPolyMask = FCP_POLY_MASK;
+// 2^x for two values on the FMA pipe (packed fp32x2): x = n + f with f in [-0.5, 0.5] by the
+// round-to-nearest magic constant, degree-3 polynomial for 2^f (max relative error 1.1e-4, well
+// below the 2^-9 of the bf16 P it feeds), exponent added as an integer.  x >= -120.
+__device__ __forceinline__ void exp2_fma(float x0, float x1, float& p0, float& p1) {
+  const f32x2 x = pack2(x0, x1);
+  const f32x2 t = add2(x, pack2(12582912.f, 12582912.f));            // 1.5 * 2^23
+  const f32x2 f = fma2(add2(t, pack2(-12582912.f, -12582912.f)), pack2(-1.f, -1.f), x);
+  f32x2 p = fma2(pack2(0.0555041086f, 0.0555041086f), f, pack2(0.2402265069f, 0.2402265069f));
+  p = fma2(p, f, pack2(0.6931471806f, 0.6931471806f));
+  p = fma2(p, f, pack2(1.0f, 1.0f));
+  float t0, t1, q0, q1;
+  unpack2(t, t0, t1);
+  unpack2(p, q0, q1);
+  p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
+  p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
+}
 constexpr float kRescaleThreshold = 8.0f;   // log2 units: rescale O only when the max grew by > 2^8
 
 template <int D, int NQ>
@@ -58,12 +86,10 @@ struct FwdCfg {
   static constexpr int kTileBytes = 128 * D * 2;           // one Q, K or V tile
   static constexpr int kPanelBytes = 128 * 128;            // 128 rows x 64 bf16
   static constexpr int kPanels = D / 64;
-  static constexpr int kPBytes = 128 * 128 * 2;            // bf16 P of one q tile: 2 panels
-  static constexpr int kStages = (D == 128) ? 3 : 6;       // ring slots, each one K or V tile
+  static constexpr int kStages = (D == 128) ? 5 : 8;       // ring slots, each one K or V tile
   static constexpr int kThreads = 128 + 128 * NQ;
   static constexpr int kTmemCols = 256 * NQ;
-  static constexpr int kOffP = NQ * kTileBytes;
-  static constexpr int kOffRing = kOffP + NQ * kPBytes;
+  static constexpr int kOffRing = NQ * kTileBytes;
   static constexpr int kSmemData = kOffRing + kStages * kTileBytes;
   static constexpr int kSmemBytes = 1024 + kSmemData + 256;
   // registers per thread after setmaxnreg (multiples of 8).  The CTA owns (launch registers x
@@ -72,17 +98,17 @@ struct FwdCfg {
   static constexpr int kRegsCtl = 72;
   static constexpr int kRegsSoftmaxRaw = (kLaunchRegs * (kThreads / 128) - kRegsCtl) / NQ / 8 * 8;
   static constexpr int kRegsSoftmax = kRegsSoftmaxRaw > 232 ? 232 : kRegsSoftmaxRaw;
-  static constexpr int kTail = 3;   // MMAs issued after the probe of the next group's barriers
 };
 static_assert(FwdCfg<128, 2>::kSmemBytes <= 232448, "fwd shared memory exceeds 227 KB");
 
 struct FwdBarriers {
   uint64_t q_full, q_empty;
   uint64_t kv_full[8], kv_empty[8];
-  uint64_t s_full[2];    // S_t written by the MMAs               -> softmax
-  uint64_t s_free[2];    // softmax holds S_t in registers         -> MMA may overwrite S_t
-  uint64_t p_ready[2];   // P_t in shared memory, O_t rescaled     -> MMA
-  uint64_t pv_done[2];   // O_t += P_t V complete: P_t smem free, O_t stable (last tile: final)
+  uint64_t s_full[2];    // S_t written by the MMAs (and, in pipe order, the O_t += P_t V before
+                         // it complete)                           -> softmax
+  uint64_t p_ready[2];   // S_t in registers, bf16 P_t written over its first 64 TMEM columns,
+                         // O_t rescaled                           -> MMA
+  uint64_t pv_done[2];   // last O_t += P_t V of the item complete -> epilogue
   uint64_t o_empty[2];   // epilogue has read O_t                  -> MMA may overwrite O_t
   uint32_t tmem_base;
 };
@@ -101,7 +127,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) &
                                              ~uintptr_t(1023));
   uint8_t* q_smem = smem;                                  // NQ tiles
-  uint8_t* p_smem = smem + Cfg::kOffP;                     // NQ tiles of bf16 P
   uint8_t* ring = smem + Cfg::kOffRing;                    // kStages tiles
   FwdBarriers* bars = reinterpret_cast<FwdBarriers*>(smem + Cfg::kSmemData);
 
@@ -117,7 +142,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     }
     for (int t = 0; t < NQ; ++t) {
       mbar_init(&bars->s_full[t], 1);
-      mbar_init(&bars->s_free[t], 128);
       mbar_init(&bars->p_ready[t], 128);
       mbar_init(&bars->pv_done[t], 1);
       mbar_init(&bars->o_empty[t], 128);
@@ -157,48 +181,48 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
           for (int pn = 0; pn < Cfg::kPanels; ++pn)
             tma_load_3d(q_smem + t * Cfg::kTileBytes + pn * Cfg::kPanelBytes, &tmap_q,
                         &bars->q_full, pn * 64, it.head0 + t, it.q_row0);
-        // consumption order of the MMAs: K0, then per tile j: K_{j+1}, V_j
+        // consumption order of the MMAs: K0, then per tile j: V_j, K_{j+1}
         load_kv(&tmap_k, it.kv_head, it.kv_row0);
         for (int j = 0; j < n; ++j) {
-          if (j + 1 < n) load_kv(&tmap_k, it.kv_head, it.kv_row0 + (j + 1) * FCP_TK);
           load_kv(&tmap_v, it.kv_head, it.kv_row0 + j * FCP_TK);
+          if (j + 1 < n) load_kv(&tmap_k, it.kv_head, it.kv_row0 + (j + 1) * FCP_TK);
         }
         iph ^= 1;
       }
     } else if (warp == 1 && elect_one()) {
       // ---------------------------------------------------------------- MMA issuer
-      // One elected thread.  Groups of 8 MMAs in the fixed order  S_t(0) | per KV tile j:
-      // S_t(j+1) for every t, then O_t += P_t(j) V_j for every t.  The barriers of the next
-      // group are probed (non-blocking) before the last kTail MMAs of the current group so the
-      // ~5-deep tcgen05 queue never drains while this thread looks at a barrier; descriptors are
-      // 32-bit adds on precomputed low words.
+      // One elected thread.  Per q tile t the chain is
+      //   S_t(0) | per KV tile j:  O_t += P_t(j) V_j  then  S_t(j+1) = Q_t K_{j+1}^T
+      // with the two tiles' chains interleaved.  P_t is the A operand straight from TMEM: the
+      // softmax warpgroup writes it (bf16) over the first 64 columns of S_t once S_t sits in
+      // registers, so S_t(j+1) must follow O_t += P_t(j) V_j in the (in-order) tensor pipe — which
+      // this issue order gives without a barrier — and the PV product reads only V from shared
+      // memory.  While tile t waits for its next S the other tile's softmax has the MUFU alone.
       constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
       constexpr uint32_t idesc_pv = umma_idesc_bf16(128, D, 0, 1);
-      constexpr int kTail = Cfg::kTail;
       constexpr int kSteps = D / 16;
       constexpr uint32_t kHi = (1024u >> 4) | (1u << 14) | (2u << 29);   // SBO, version, swizzle
       constexpr uint32_t kTileStep = Cfg::kTileBytes >> 4;
       auto lo_word = [](uint32_t saddr, uint32_t lbo) { return ((saddr & 0x3FFFF) >> 4) | ((lbo >> 4) << 16); };
       auto desc = [](uint32_t lo) { return ((uint64_t)kHi << 32) | lo; };
       const uint32_t q_kmaj = lo_word(smem_u32(q_smem), 16);                     // A of S (tile 0)
-      const uint32_t p_kmaj = lo_word(smem_u32(p_smem), 16);                     // A of O (tile 0)
       const uint32_t ring_kmaj = lo_word(smem_u32(ring), 16);                    // K tile, slot 0
       const uint32_t ring_mnmaj = lo_word(smem_u32(ring), Cfg::kPanelBytes);     // V tile, slot 0
 
-      auto issue_qk = [&](int t, uint32_t kslot, int kk0, int kk1) {
+      auto issue_qk = [&](int t, uint32_t kslot) {
         const uint32_t a0 = q_kmaj + t * kTileStep, b0 = ring_kmaj + kslot * kTileStep;
 #pragma unroll
-        for (int kk = kk0; kk < kk1; ++kk) {
+        for (int kk = 0; kk < kSteps; ++kk) {
           const uint32_t off = ((kk >> 2) * Cfg::kPanelBytes + (kk & 3) * 32) >> 4;
           umma_ss(tmem_base + t * 128, desc(a0 + off), desc(b0 + off), idesc_qk, kk > 0);
         }
       };
-      auto issue_pv = [&](int t, uint32_t vslot, bool acc, int kk0, int kk1) {
-        const uint32_t a0 = p_kmaj + t * (Cfg::kPBytes >> 4), b0 = ring_mnmaj + vslot * kTileStep;
+      // A = P_t from TMEM: 16 keys of bf16 = 8 columns per K step
+      auto issue_pv = [&](int t, uint32_t vslot, bool acc) {
+        const uint32_t b0 = ring_mnmaj + vslot * kTileStep;
 #pragma unroll
-        for (int kk = kk0; kk < kk1; ++kk)
-          umma_ss(tmem_base + (NQ + t) * 128,
-                  desc(a0 + (((kk >> 2) * Cfg::kPanelBytes + (kk & 3) * 32) >> 4)),
+        for (int kk = 0; kk < 8; ++kk)
+          umma_ts(tmem_base + (NQ + t) * 128, tmem_base + t * 128 + kk * 8,
                   desc(b0 + kk * (2048 >> 4)), idesc_pv, (acc || kk > 0) ? 1u : 0u);
       };
       auto ring_next = [](uint32_t& s_, uint32_t& p_) {
@@ -206,9 +230,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       };
 
       uint32_t slot = 0, sph = 0;      // ring position / phase parity of the next tile to consume
-      uint32_t sfp[NQ], ppp[NQ];       // parities: S_t free (starts "already free"), P_t ready
-#pragma unroll
-      for (int t = 0; t < NQ; ++t) { sfp[t] = 1; ppp[t] = 0; }
+      uint32_t ppp = 0;                // parity of p_ready (both tiles advance together)
       uint32_t iph = 0;                // item parity (q_full; o_empty of the previous item)
 #ifdef FCP_EXP_TRACE
       uint32_t tn = 0;
@@ -217,83 +239,51 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       for (int idx = item_begin; idx < item_end; ++idx) {
         const int n = items[idx].n_kv_tiles;
         if (n == 0) continue;
-        // probes of the group that follows: S_t (tile jq) or O_t (tile jp) on ring slot (s_, p_)
-        auto test_qk = [&](int t, uint32_t s_, uint32_t p_) -> bool {
-          return mbar_test(&bars->s_free[t], sfp[t]) & (t > 0 || mbar_test(&bars->kv_full[s_], p_));
-        };
-        auto test_pv = [&](int t, uint32_t s_, uint32_t p_, int j) -> bool {
-          return mbar_test(&bars->p_ready[t], ppp[t]) & (t > 0 || mbar_test(&bars->kv_full[s_], p_)) &
-                 (j > 0 || mbar_test(&bars->o_empty[t], iph ^ 1));
-        };
         mbar_wait(&bars->q_full, iph);
         mbar_wait(&bars->kv_full[slot], sph);
+        tc_fence_after();
 #pragma unroll
         for (int t = 0; t < NQ; ++t) {
-          mbar_wait(&bars->s_free[t], sfp[t]);
-          sfp[t] ^= 1;
-          tc_fence_after();
-          issue_qk(t, slot, 0, kSteps);
+          // S_t is free: the previous item's last P_t V was issued before (in-order pipe)
+          issue_qk(t, slot);
           umma_commit(&bars->s_full[t]);
         }
         umma_commit(&bars->kv_empty[slot]);
         if (n == 1) umma_commit(&bars->q_empty);
         ring_next(slot, sph);
-        bool ok = false;               // barriers of the upcoming group already seen complete
         for (int j = 0; j < n; ++j) {
           const bool has_next = j + 1 < n;
-          if (has_next) {
-            // ---- S_t(j+1) = Q_t K_{j+1}^T
-#pragma unroll
-            for (int t = 0; t < NQ; ++t) {
-              if (!ok) {
-                if (t == 0) mbar_wait(&bars->kv_full[slot], sph);
-                mbar_wait(&bars->s_free[t], sfp[t]);
-              }
-              sfp[t] ^= 1;
-              tc_fence_after();
-              issue_qk(t, slot, 0, kSteps - kTail);
-              if (t + 1 < NQ) {
-                ok = test_qk(t + 1 < NQ ? t + 1 : 0, slot, sph);
-              } else {
-                uint32_t s1 = slot, p1 = sph;
-                ring_next(s1, p1);
-                ok = test_pv(0, s1, p1, j);
-              }
-              issue_qk(t, slot, kSteps - kTail, kSteps);
-              umma_commit(&bars->s_full[t]);
-            }
-            umma_commit(&bars->kv_empty[slot]);
-            if (j + 2 == n) umma_commit(&bars->q_empty);
-            ring_next(slot, sph);
-          }
-          // ---- O_t += P_t(j) V_j
+          const uint32_t vslot = slot, vph = sph;
+          uint32_t kslot = slot, kph = sph;
+          ring_next(kslot, kph);                    // K_{j+1} follows V_j in the ring
 #pragma unroll
           for (int t = 0; t < NQ; ++t) {
             FTRACE(tn, 8 + 3 * t);
-            if (!ok) {
-              if (t == 0) mbar_wait(&bars->kv_full[slot], sph);
-              if (j == 0) mbar_wait(&bars->o_empty[t], iph ^ 1);
-              mbar_wait(&bars->p_ready[t], ppp[t]);
-            }
+            if (t == 0) mbar_wait(&bars->kv_full[vslot], vph);
+            if (j == 0) mbar_wait(&bars->o_empty[t], iph ^ 1);
+            mbar_wait(&bars->p_ready[t], ppp);
             FTRACE(tn, 9 + 3 * t);
-            ppp[t] ^= 1;
             tc_fence_after();
-            issue_pv(t, slot, j > 0, 0, 8 - kTail);
-            if (t + 1 < NQ) {
-              ok = test_pv(t + 1 < NQ ? t + 1 : 0, slot, sph, j);
-            } else if (has_next) {
-              uint32_t s1 = slot, p1 = sph;
-              ring_next(s1, p1);
-              ok = (j + 2 < n) ? test_qk(0, s1, p1) : test_pv(0, s1, p1, j + 1);
-            } else {
-              ok = false;              // next item: blocking waits
+            issue_pv(t, vslot, j > 0);
+            if (!has_next) umma_commit(&bars->pv_done[t]);
+            if (has_next) {
+              if (t == 0) {
+                mbar_wait(&bars->kv_full[kslot], kph);
+                tc_fence_after();
+              }
+              issue_qk(t, kslot);
+              umma_commit(&bars->s_full[t]);
             }
-            issue_pv(t, slot, true, 8 - kTail, 8);
-            umma_commit(&bars->pv_done[t]);
             FTRACE(tn, 10 + 3 * t);
           }
-          umma_commit(&bars->kv_empty[slot]);
+          ppp ^= 1;
+          umma_commit(&bars->kv_empty[vslot]);
           ring_next(slot, sph);
+          if (has_next) {
+            umma_commit(&bars->kv_empty[kslot]);
+            if (j + 2 == n) umma_commit(&bars->q_empty);
+            ring_next(slot, sph);
+          }
 #ifdef FCP_EXP_TRACE
           ++tn;
 #endif
@@ -318,8 +308,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t tS = tmem_base + lane_addr + t * 128;
     const uint32_t tO = tmem_base + lane_addr + (NQ + t) * 128;
-    const uint32_t p_row_addr = smem_u32(p_smem) + t * Cfg::kPBytes + row * 128;
-    const uint32_t swz = row & 7;
     uint32_t s_ph = 0, pv_ph = 0;
 #ifdef FCP_EXP_TRACE
     uint32_t tn = 0;
@@ -355,8 +343,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, sr[c]);
         tmem_ld_wait();
-        tc_fence_before();
-        mbar_arrive(&bars->s_free[t]);              // S_t(j+1) may now overwrite S_t
         if ((warp & 3) == 0) FTRACE(tn, 4 * t + 2);
         const int col0 = j * FCP_TK;
         if (col0 + FCP_TK - 1 > warp_min_limit) {   // diagonal / boundary tile: mask in registers
@@ -378,7 +364,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
         // p = exp2(s c - m_ref) for the whole row, packed to bf16; returns the row sum.  Packed
         // fp32x2 FMA / ADD and the 3-input max keep the loop MUFU-bound (6 issue slots per 2
         // elements of which 2 are MUFU).
-        bool pv_waited = j == 0;     // first tile of the item: P_t and O_t are free (epilogue waited)
         bool token_passed = NQ != 2 || kTokenQuarter < 0;
         auto exp_row = [&](float m_ref, float& mx_out, bool with_max) -> float {
           const f32x2 negm2 = pack2(-m_ref, -m_ref);
@@ -397,27 +382,25 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
               float x0, x1, x2, x3;
               unpack2(fma2(pack2(s0, s1), scale2, negm2), x0, x1);
               unpack2(fma2(pack2(s2, s3), scale2, negm2), x2, x3);
-              const float p0 = fast_exp2(x0), p1 = fast_exp2(x1), p2 = fast_exp2(x2), p3 = fast_exp2(x3);
+              const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
+              float p2, p3;
+              // fast path only: every row of the warp has a finite running max there, so a masked
+              // score may come out as 2^-120 instead of 0 without changing l or O
+              if (with_max && ((kPolyMask >> (i >> 1)) & 1u)) {
+                exp2_fma(fmaxf(x2, -120.f), fmaxf(x3, -120.f), p2, p3);
+              } else {
+                p2 = fast_exp2(x2);
+                p3 = fast_exp2(x3);
+              }
               sum_a = add2(sum_a, pack2(p0, p1));
               sum_b = add2(sum_b, pack2(p2, p3));
               pk[c * 16 + i] = pack_bf16(p0, p1);
               pk[c * 16 + i + 1] = pack_bf16(p2, p3);
             }
-            // The previous O_t += P V must have finished before P_t is overwritten (it reads P
-            // from shared memory); one quarter of the exponentials later it normally has.
-            if (!pv_waited) {
-              mbar_wait(&bars->pv_done[t], pv_ph);
-              pv_ph ^= 1;
-              tc_fence_after();
-              pv_waited = true;
-            }
-            // this quarter of the P row: 4 swizzled 16-byte chunks (K-major SWIZZLE_128B operand)
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              const int ch = c * 4 + q;
-              sts128(p_row_addr + (ch >> 3) * Cfg::kPanelBytes + (((ch & 7) ^ swz) << 4),
-                     pk[4 * ch], pk[4 * ch + 1], pk[4 * ch + 2], pk[4 * ch + 3]);
-            }
+            // this quarter of the P row (32 keys = 16 bf16 pairs) goes over the first columns of
+            // S_t — the whole of S_t is in registers, and the previous O_t += P V finished before
+            // S_t was written (same pipe, issued earlier)
+            tmem_st16(tS + c * 16, *reinterpret_cast<const uint32_t(*)[16]>(&pk[c * 16]));
             // hand the MUFU token on part-way: the other tile starts its exponentials while
             // this one finishes (two warps per sub-partition keep the MUFU saturated; one alone
             // is latency-bound)
@@ -470,9 +453,8 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
             for (int i = 0; i < 32; ++i) orow[i] = __float_as_uint(__uint_as_float(orow[i]) * alpha);
             tmem_st32(tO + c * 32, orow);
           }
-          tmem_st_wait();
         }
-        fence_proxy_async_smem();
+        tmem_st_wait();
         tc_fence_before();
         mbar_arrive(&bars->p_ready[t]);
         if ((warp & 3) == 0) FTRACE(tn, 4 * t + 3);

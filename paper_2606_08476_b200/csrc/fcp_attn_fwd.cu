@@ -11,7 +11,7 @@
 // two from exponentiating at the same time: two warps per sub-partition in lockstep idle the
 // MUFU during their loads and stores).
 //
-//   warp 0      TMA producer   Q (once per item); K/V tiles through a 5-slot ring in the order
+//   warp 0      TMA producer   Q (once per item); K/V tiles through a 3-slot ring in the order
 //                              the MMAs consume them: K0, V0, K1, V1, ...
 //   warp 1      MMA issuer     one elected thread; per KV tile j and q tile t: O_t += P_t(j) V_j
 //                              (A = P from TMEM, B = V MN-major), then S_t(j+1) (SS) — program
@@ -79,18 +79,30 @@ __device__ __forceinline__ void exp2_fma(float x0, float x1, float& p0, float& p
   p0 = __int_as_float(__float_as_int(q0) + (__float_as_int(t0) << 23));
   p1 = __int_as_float(__float_as_int(q1) + (__float_as_int(t1) << 23));
 }
-constexpr float kRescaleThreshold = 8.0f;   // log2 units: rescale O only when the max grew by > 2^8
+constexpr float kRescaleThreshold = 8.0f;
+
+// 3-D tiled store shared -> global through a tensor map (coordinates as tma_load_3d)
+__device__ __forceinline__ void tma_store_3d(const void* tmap, const void* smem_src, int32_t c0,
+                                             int32_t c1, int32_t c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::
+                   "l"(tmap), "r"(smem_u32(smem_src)), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }   // log2 units: rescale O only when the max grew by > 2^8
 
 template <int D, int NQ>
 struct FwdCfg {
   static constexpr int kTileBytes = 128 * D * 2;           // one Q, K or V tile
   static constexpr int kPanelBytes = 128 * 128;            // 128 rows x 64 bf16
   static constexpr int kPanels = D / 64;
-  static constexpr int kStages = (D == 128) ? 5 : 8;       // ring slots, each one K or V tile
+  static constexpr int kStages = (D == 128) ? 3 : 6;       // ring slots, each one K or V tile
   static constexpr int kThreads = 128 + 128 * NQ;
   static constexpr int kTmemCols = 256 * NQ;
   static constexpr int kOffRing = NQ * kTileBytes;
-  static constexpr int kSmemData = kOffRing + kStages * kTileBytes;
+  static constexpr int kOffOut = kOffRing + kStages * kTileBytes;   // NQ staging tiles for o
+  static constexpr int kSmemData = kOffOut + NQ * kTileBytes;
   static constexpr int kSmemBytes = 1024 + kSmemData + 256;
   // registers per thread after setmaxnreg (multiples of 8).  The CTA owns (launch registers x
   // threads): the sum over its warpgroups must stay below.
@@ -119,6 +131,7 @@ __global__ void __launch_bounds__(FwdCfg<D, NQ>::kThreads, 1)
 fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
                     const __grid_constant__ CUtensorMap tmap_k,
                     const __grid_constant__ CUtensorMap tmap_v,
+                    const __grid_constant__ CUtensorMap tmap_o,
                     const FwdItem* __restrict__ items, const int32_t* __restrict__ cta_off,
                     __nv_bfloat16* __restrict__ o, float* __restrict__ lse,
                     int64_t n_q, int Hq, float scale_log2) {
@@ -128,6 +141,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
                                              ~uintptr_t(1023));
   uint8_t* q_smem = smem;                                  // NQ tiles
   uint8_t* ring = smem + Cfg::kOffRing;                    // kStages tiles
+  uint8_t* out_smem = smem + Cfg::kOffOut;                 // NQ tiles: o rows staged for the TMA store
   FwdBarriers* bars = reinterpret_cast<FwdBarriers*>(smem + Cfg::kSmemData);
 
   const int warp = threadIdx.x >> 5;
@@ -266,6 +280,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
             tc_fence_after();
             issue_pv(t, vslot, j > 0);
             if (!has_next) umma_commit(&bars->pv_done[t]);
+            if (t == NQ - 1) umma_commit(&bars->kv_empty[vslot]);   // V_j: both tiles have read it
             if (has_next) {
               if (t == 0) {
                 mbar_wait(&bars->kv_full[kslot], kph);
@@ -277,7 +292,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
             FTRACE(tn, 10 + 3 * t);
           }
           ppp ^= 1;
-          umma_commit(&bars->kv_empty[vslot]);
           ring_next(slot, sph);
           if (has_next) {
             umma_commit(&bars->kv_empty[kslot]);
@@ -313,9 +327,12 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     uint32_t tn = 0;
 #endif
     if (NQ == 2 && t == 1) named_bar_arrive(2, 256);        // tile 0 holds the MUFU token first
+    const bool o_al32 = (reinterpret_cast<uintptr_t>(o) & 31) == 0;
+    FwdItem nxt;
+    if (item_begin < item_end) nxt = items[item_begin];
 
     for (int idx = item_begin; idx < item_end; ++idx) {
-      const FwdItem it = items[idx];
+      const FwdItem it = nxt;
       const int n = it.n_kv_tiles;
       const int head = it.head0 + t;
       const bool row_valid = row < it.q_rows;
@@ -326,6 +343,7 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
           for (int c = 0; c < D; c += 8) *reinterpret_cast<int4*>(o_row + c) = make_int4(0, 0, 0, 0);
           *lse_row = -INFINITY;
         }
+        if (idx + 1 < item_end) nxt = items[idx + 1];
         continue;
       }
       // last visible key (segment position) of this row; may be negative
@@ -467,29 +485,73 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       mbar_wait(&bars->pv_done[t], pv_ph);
       pv_ph ^= 1;
       tc_fence_after();
+      if ((warp & 3) == 0 && t == 0) FTRACE(tn - 1, 14);
       const float inv = l > 0.f ? 1.f / l : 0.f;
+      // The whole O row leaves TMEM first: O_t is free for the next item's first PV product at
+      // once, and the loads do not queue behind the store burst below.
+      uint32_t orow[D / 32][32];
 #pragma unroll
-      for (int c = 0; c < D / 32; ++c) {
-        uint32_t orow[32];
-        tmem_ld32(tO + c * 32, orow);
-        tmem_ld_wait();
-        if (row_valid) {
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            int4 v;
-            v.x = pack_bf16(__uint_as_float(orow[8 * i + 0]) * inv, __uint_as_float(orow[8 * i + 1]) * inv);
-            v.y = pack_bf16(__uint_as_float(orow[8 * i + 2]) * inv, __uint_as_float(orow[8 * i + 3]) * inv);
-            v.z = pack_bf16(__uint_as_float(orow[8 * i + 4]) * inv, __uint_as_float(orow[8 * i + 5]) * inv);
-            v.w = pack_bf16(__uint_as_float(orow[8 * i + 6]) * inv, __uint_as_float(orow[8 * i + 7]) * inv);
-            *reinterpret_cast<int4*>(o_row + c * 32 + i * 8) = v;
-          }
-        }
-      }
+      for (int c = 0; c < D / 32; ++c) tmem_ld32(tO + c * 32, orow[c]);
+      tmem_ld_wait();
       tc_fence_before();
       mbar_arrive(&bars->o_empty[t]);
+      // next item's descriptor: issued before the stores so that it does not wait behind them
+      if (idx + 1 < item_end) nxt = items[idx + 1];
+      if (it.q_rows == FCP_TQ) {
+        // Full tile: rows are staged in shared memory in the SWIZZLE_128B layout of the o tensor
+        // map and leave with one TMA store per 64-column panel (a thread owns a row, so direct
+        // stores would touch 32 lines per instruction and back up the LSU for ~2000 clocks).
+        const bool issuer = (warp & 3) == 0 && lane == 0;
+        if (issuer) bulk_wait_read0();                 // the previous item's store has read the tile
+        named_bar_sync(4 + t, 128);
+        const uint32_t out_row = smem_u32(out_smem) + t * Cfg::kTileBytes + row * 128;
+        const uint32_t swz = row & 7;
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c)
+#pragma unroll
+          for (int i = 0; i < 4; ++i) {
+            const int ch = c * 4 + i;                  // 16-byte chunk of the row
+            sts128(out_row + (ch >> 3) * Cfg::kPanelBytes + (((ch & 7) ^ swz) << 4),
+                   pack_bf16(__uint_as_float(orow[c][8 * i + 0]) * inv, __uint_as_float(orow[c][8 * i + 1]) * inv),
+                   pack_bf16(__uint_as_float(orow[c][8 * i + 2]) * inv, __uint_as_float(orow[c][8 * i + 3]) * inv),
+                   pack_bf16(__uint_as_float(orow[c][8 * i + 4]) * inv, __uint_as_float(orow[c][8 * i + 5]) * inv),
+                   pack_bf16(__uint_as_float(orow[c][8 * i + 6]) * inv, __uint_as_float(orow[c][8 * i + 7]) * inv));
+          }
+        fence_proxy_async_smem();
+        named_bar_sync(4 + t, 128);
+        if (issuer) {
+#pragma unroll
+          for (int pn = 0; pn < Cfg::kPanels; ++pn)
+            tma_store_3d(&tmap_o, out_smem + t * Cfg::kTileBytes + pn * Cfg::kPanelBytes, pn * 64,
+                         head, it.q_row0);
+          bulk_commit();
+        }
+      } else if (row_valid) {
+        // ragged last tile of a shard: the rows after it belong to another shard, so each thread
+        // stores its own row (32-byte stores when o is 32-byte aligned)
+#pragma unroll
+        for (int c = 0; c < D / 32; ++c)
+#pragma unroll
+          for (int i = 0; i < 2; ++i) {
+            uint32_t w[8];
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+              w[k] = pack_bf16(__uint_as_float(orow[c][16 * i + 2 * k]) * inv,
+                               __uint_as_float(orow[c][16 * i + 2 * k + 1]) * inv);
+            __nv_bfloat16* dst = o_row + c * 32 + i * 16;
+            if (o_al32) {
+              stg256(dst, w);
+            } else {
+              *reinterpret_cast<int4*>(dst) = make_int4(w[0], w[1], w[2], w[3]);
+              *reinterpret_cast<int4*>(dst + 8) = make_int4(w[4], w[5], w[6], w[7]);
+            }
+          }
+      }
       if (row_valid) *lse_row = l > 0.f ? kLn2 * (m + __log2f(l)) : -INFINITY;
+      if ((warp & 3) == 0 && t == 0) FTRACE(tn - 1, 15);
     }
     if (NQ == 2 && t == 0) named_bar_sync(2, 256);          // consume tile 1's last token
+    if ((warp & 3) == 0 && lane == 0) bulk_wait0();         // o stores of the last item
   }
 
   tc_fence_before();
@@ -503,14 +565,15 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
 template <int D, int NQ>
 int launch_fwd(const fcp_attn_args* a, const fcp_sched* s) {
   using Cfg = FwdCfg<D, NQ>;
-  CUtensorMap mq, mk, mv;
+  CUtensorMap mq, mk, mv, mo;
   // an empty KV buffer (n_kv == 0: a PREFIX piece of shards that all start their document) has
   // no tile to load; its maps only need a valid base
   const void* kb = s->n_kv > 0 ? a->k : a->q;
   const void* vb = s->n_kv > 0 ? a->v : a->q;
   if (!make_tmap_rows(&mq, a->q, D, s->Hq, s->n_q, 128) ||
       !make_tmap_rows(&mk, kb, D, s->Hkv, s->n_kv, 128) ||
-      !make_tmap_rows(&mv, vb, D, s->Hkv, s->n_kv, 128))
+      !make_tmap_rows(&mv, vb, D, s->Hkv, s->n_kv, 128) ||
+      !make_tmap_rows(&mo, a->o, D, s->Hq, s->n_q, 128))
     return FCP_CUDA;
   auto kern = fcp_attn_fwd_kernel<D, NQ>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes) !=
@@ -522,7 +585,7 @@ int launch_fwd(const fcp_attn_args* a, const fcp_sched* s) {
   cudaStream_t st = (cudaStream_t)a->stream;
   if (a->ev_start && cudaEventRecord((cudaEvent_t)a->ev_start, st) != cudaSuccess) return FCP_CUDA;
   kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(
-      mq, mk, mv, items,
+      mq, mk, mv, mo, items,
       reinterpret_cast<const int32_t*>(static_cast<const char*>(a->workspace) + s->off_fwd_cta),
       static_cast<__nv_bfloat16*>(a->o), a->lse, s->n_q, s->Hq, a->scale * kLog2e);
   if (cudaGetLastError() != cudaSuccess) return FCP_CUDA;

@@ -240,6 +240,13 @@ __device__ __forceinline__ void tmem_st_wait() {
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
+// 32-byte global store (address 32-byte aligned): one full L2 sector per lane
+__device__ __forceinline__ void stg256(void* gptr, const uint32_t (&w)[8]) {
+  asm volatile("st.global.v8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(gptr), "r"(w[0]),
+               "r"(w[1]), "r"(w[2]), "r"(w[3]), "r"(w[4]), "r"(w[5]), "r"(w[6]), "r"(w[7])
+               : "memory");
+}
+
 // ---------------------------------------------------------------- shared-memory accesses by address
 // (explicit .shared state space: the compiler cannot always prove it and would emit generic LD/ST)
 __device__ __forceinline__ float4 lds128(uint32_t saddr) {

@@ -414,6 +414,34 @@ def test_outputs_do_not_write_out_of_bounds(fcp, torch):
         assert not bool((lse == CAN).any())
 
 
+def test_sixteen_byte_aligned_outputs(fcp, torch):
+    """include/fcp.h promises 16-byte alignment is enough.  The forward stores o through a TMA
+    tensor map (full tiles) or with 32-byte stores when the base allows it (ragged tiles): an o
+    that is 16- but not 32-byte aligned must take the 16-byte path and give the same bits; an
+    8-byte offset is FCP_MISALIGNED."""
+    d, N, Hq, Hkv, D = [333, 77, 130, 1, 63, 36], 2, 4, 2, 128
+    scale = 1.0 / math.sqrt(D)
+    Q, K, V, dO = fcp_inputs.make_tensors(sum(d), Hq, Hkv, D, 4)
+    plan = fcp.Plan(d, N)
+    lay = plan.rank_layout(0)
+    qi = torch.from_numpy(lay["q_token_index"].astype(np.int64))
+    q = Q[qi].contiguous().cuda()
+    kg, vg, _ = plan.kv_gather(0, K.cuda(), V.cuda())
+    sched = plan.sched(0, Hq, Hkv, D).upload("cuda")
+    o_ref, lse_ref = sched.attn_fwd(q, kg, vg, scale)
+    flat = torch.zeros(q.numel() + 64, dtype=torch.bfloat16, device="cuda")
+    assert flat.data_ptr() % 32 == 0
+    o16 = flat[8:8 + q.numel()].view(q.shape)             # +16 bytes
+    assert o16.data_ptr() % 32 == 16
+    o_got, lse_got = sched.attn_fwd(q, kg, vg, scale, o=o16)
+    torch.cuda.synchronize()
+    assert torch.equal(o_got, o_ref) and torch.equal(lse_got, lse_ref)
+    assert bool((flat[:8] == 0).all()) and bool((flat[8 + q.numel():] == 0).all())
+    o8 = flat[4:4 + q.numel()].view(q.shape)               # +8 bytes
+    with pytest.raises(fcp.FcpError):
+        sched.attn_fwd(q, kg, vg, scale, o=o8)
+
+
 def test_missing_library_fails_loudly(fcp, monkeypatch):
     import paper_2606_08476_b200.binding as B
     monkeypatch.setattr(B, "_LIB", None)

@@ -199,6 +199,13 @@ __device__ __forceinline__ void bulk_reduce_add_f32(float* gdst, const void* ssr
       "r"(smem_u32(ssrc)), "r"(bytes)
       : "memory");
 }
+// 3-D tiled store shared -> global through a tensor map (coordinates as tma_load_3d)
+__device__ __forceinline__ void tma_store_3d(const void* tmap, uint32_t smem_src, int32_t c0,
+                                             int32_t c1, int32_t c2) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];" ::
+                   "l"(tmap), "r"(smem_src), "r"(c0), "r"(c1), "r"(c2)
+               : "memory");
+}
 __device__ __forceinline__ void bulk_commit() {
   asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
@@ -256,6 +263,8 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
                   const __grid_constant__ CUtensorMap tmap_do,
                   const __grid_constant__ CUtensorMap tmap_k,
                   const __grid_constant__ CUtensorMap tmap_v,
+                  const __grid_constant__ CUtensorMap tmap_dk,
+                  const __grid_constant__ CUtensorMap tmap_dv,
                   const BwdItem* __restrict__ items, const int32_t* __restrict__ cta_off,
                   const BwdSub* __restrict__ subs, const float2* __restrict__ lsed,
                   float* __restrict__ dq_acc, void* __restrict__ dk_out,
@@ -487,6 +496,8 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
     const uint32_t stat_base = smem_u32(stat_smem) + half * 32 * 8;
     const uint32_t ds_base = smem_u32(ds_smem) + row * 128;
+    const bool issuer = (warp & 3) == 0 && lane == 0;  // one thread per warpgroup issues its TMA stores
+    bool staged = false;
     uint32_t n = 0, m = 0;
     for (int idx = item_begin; idx < item_end; ++idx) {
       const BwdItem it = items[idx];
@@ -502,6 +513,13 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       }
       const int kv_pos = it.kv_pos0 + row;
       const int warp_kv_max = it.kv_pos0 + (warp & 3) * 32 + 31;
+      if (staged) {
+        // the previous item's dk / dv left through the dS^T buffers: both stores must have read
+        // them before any softmax thread writes dS^T again
+        if (issuer) bulk_wait_read0();
+        named_bar_sync(6, 256);
+        staged = false;
+      }
       for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
         const uint32_t st = n % Cfg::kStages;
         const uint32_t tS = tmem_base + lane_addr + Cfg::kColS + (n & 1) * 64;
@@ -543,34 +561,74 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         const uint32_t tacc = tmem_base + lane_addr + (half == 0 ? Cfg::kColDV : Cfg::kColDK);
         const float f = half == 0 ? 1.f : scale;
         __nv_bfloat16* dst = reinterpret_cast<__nv_bfloat16*>(dst_b);
+        if (!dkv_f32 && it.kv_rows == 128) {
+          // Full bf16 tile: the accumulator rows leave TMEM first (dV / dK are free for the next
+          // item at once), then go panel by panel (64 columns = 128 B per row) through this
+          // warpgroup's dS^T buffer — idle between items — in the SWIZZLE_128B layout of the
+          // dk / dv tensor map, one TMA store per panel.  A thread owns a row: direct stores touch
+          // 32 lines per instruction and back the LSU up in front of the next item's loads.
+          uint32_t acc[D / 32][32];
 #pragma unroll
-        for (int c = 0; c < D / 32; ++c) {
-          uint32_t acc[32];
-          tmem_ld32(tacc + c * 32, acc);
+          for (int c = 0; c < D / 32; ++c) tmem_ld32(tacc + c * 32, acc[c]);
           tmem_ld_wait();
-          if (row_valid && dkv_f32) {
-            float4* d4 = reinterpret_cast<float4*>(dst_b) + c * 8;
+          tc_fence_before();
+          mbar_arrive(&bars->dkv_free);
+          const uint32_t stage = smem_u32(ds_smem) + half * Cfg::kDS;
+          const uint32_t stage_row = stage + row * 128;
+          const uint32_t swz = row & 7;
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
-              d4[i] = make_float4(__uint_as_float(acc[4 * i + 0]) * f, __uint_as_float(acc[4 * i + 1]) * f,
-                                  __uint_as_float(acc[4 * i + 2]) * f, __uint_as_float(acc[4 * i + 3]) * f);
-          } else if (row_valid) {
+          for (int pn = 0; pn < Cfg::kPanels; ++pn) {
+            if (pn > 0 && issuer) bulk_wait_read0();    // the previous panel has been read
+            if (pn > 0) named_bar_sync(4 + half, 128);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-              int4 pk;
-              pk.x = pack_bf16(__uint_as_float(acc[8 * i + 0]) * f, __uint_as_float(acc[8 * i + 1]) * f);
-              pk.y = pack_bf16(__uint_as_float(acc[8 * i + 2]) * f, __uint_as_float(acc[8 * i + 3]) * f);
-              pk.z = pack_bf16(__uint_as_float(acc[8 * i + 4]) * f, __uint_as_float(acc[8 * i + 5]) * f);
-              pk.w = pack_bf16(__uint_as_float(acc[8 * i + 6]) * f, __uint_as_float(acc[8 * i + 7]) * f);
-              *reinterpret_cast<int4*>(dst + c * 32 + i * 8) = pk;
+            for (int ch = 0; ch < 8; ++ch) {
+              const int e = (ch & 3) * 8;               // element inside the 32-column chunk
+              const uint32_t* a = acc[pn * 2 + (ch >> 2)];
+              sts128(stage_row + ((ch ^ swz) << 4),
+                     pack_bf16(__uint_as_float(a[e + 0]) * f, __uint_as_float(a[e + 1]) * f),
+                     pack_bf16(__uint_as_float(a[e + 2]) * f, __uint_as_float(a[e + 3]) * f),
+                     pack_bf16(__uint_as_float(a[e + 4]) * f, __uint_as_float(a[e + 5]) * f),
+                     pack_bf16(__uint_as_float(a[e + 6]) * f, __uint_as_float(a[e + 7]) * f));
+            }
+            fence_proxy_async_smem();
+            named_bar_sync(4 + half, 128);
+            if (issuer) {
+              tma_store_3d(half == 0 ? &tmap_dv : &tmap_dk, stage, pn * 64, it.kv_head, it.kv_row0);
+              bulk_commit();
             }
           }
+          staged = true;
+        } else {
+#pragma unroll
+          for (int c = 0; c < D / 32; ++c) {
+            uint32_t acc[32];
+            tmem_ld32(tacc + c * 32, acc);
+            tmem_ld_wait();
+            if (row_valid && dkv_f32) {
+              float4* d4 = reinterpret_cast<float4*>(dst_b) + c * 8;
+#pragma unroll
+              for (int i = 0; i < 8; ++i)
+                d4[i] = make_float4(__uint_as_float(acc[4 * i + 0]) * f, __uint_as_float(acc[4 * i + 1]) * f,
+                                    __uint_as_float(acc[4 * i + 2]) * f, __uint_as_float(acc[4 * i + 3]) * f);
+            } else if (row_valid) {
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                int4 pk;
+                pk.x = pack_bf16(__uint_as_float(acc[8 * i + 0]) * f, __uint_as_float(acc[8 * i + 1]) * f);
+                pk.y = pack_bf16(__uint_as_float(acc[8 * i + 2]) * f, __uint_as_float(acc[8 * i + 3]) * f);
+                pk.z = pack_bf16(__uint_as_float(acc[8 * i + 4]) * f, __uint_as_float(acc[8 * i + 5]) * f);
+                pk.w = pack_bf16(__uint_as_float(acc[8 * i + 6]) * f, __uint_as_float(acc[8 * i + 7]) * f);
+                *reinterpret_cast<int4*>(dst + c * 32 + i * 8) = pk;
+              }
+            }
+          }
+          tc_fence_before();
+          mbar_arrive(&bars->dkv_free);
         }
       }
-      tc_fence_before();
-      mbar_arrive(&bars->dkv_free);
       ++m;
     }
+    if (issuer) bulk_wait0();                          // dk / dv stores of the last item
   } else {
     // ------------------------------------------------------------------ dQ drain (warps 12-15)
     reg_dealloc<Cfg::kRegsDrain>();
@@ -645,11 +703,16 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
   }
   const int n_items = (int)s->bwd.size();
   if (n_items > 0) {
-    CUtensorMap mq, mdo, mk, mv;
+    CUtensorMap mq, mdo, mk, mv, mdk, mdv;
     if (!make_tmap_rows(&mq, a->q, D, s->Hq, s->n_q, FCP_BQ) ||
         !make_tmap_rows(&mdo, dO, D, s->Hq, s->n_q, FCP_BQ) ||
         !make_tmap_rows(&mk, a->k, D, s->Hkv, s->n_kv, 128) ||
         !make_tmap_rows(&mv, a->v, D, s->Hkv, s->n_kv, 128))
+      return FCP_CUDA;
+    // bf16 dk / dv leave through TMA stores; fp32 partials are stored row by row (maps unused)
+    const bool f32 = a->dkv_dtype == FCP_DTYPE_F32;
+    if (!make_tmap_rows(&mdk, f32 ? a->k : dk, D, s->Hkv, s->n_kv, 128) ||
+        !make_tmap_rows(&mdv, f32 ? a->v : dv, D, s->Hkv, s->n_kv, 128))
       return FCP_CUDA;
     auto kern = fcp_attn_bwd_main<D>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -659,7 +722,7 @@ int launch_bwd(const fcp_attn_args* a, const fcp_sched* s, const void* dO, void*
     if (a->ev_start && cudaEventRecord((cudaEvent_t)a->ev_start, st) != cudaSuccess)
       return FCP_CUDA;
     kern<<<grid, Cfg::kThreads, Cfg::kSmemBytes, st>>>(
-        mq, mdo, mk, mv, reinterpret_cast<const BwdItem*>(ws + s->off_bwd),
+        mq, mdo, mk, mv, mdk, mdv, reinterpret_cast<const BwdItem*>(ws + s->off_bwd),
         reinterpret_cast<const int32_t*>(ws + s->off_bwd_cta),
         reinterpret_cast<const BwdSub*>(ws + s->off_sub), lsed, dq_acc, dk, dv,
         a->dkv_dtype == FCP_DTYPE_F32, s->n_q_pad, s->Hkv, s->G, a->scale, a->scale * kLog2e);

@@ -556,7 +556,7 @@ def run_fcp(args):
         kv_b = 2 * row_bytes                                  # K and V, one pass, per token
         # dram__bytes_read + dram__bytes_write of the dominant kernel from the committed ncu capture
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "r1d_traffic.csv")
+        tp = os.path.join(ROOT, "profiles", "r1g_traffic.csv")
         if os.path.exists(tp):
             try:
                 import csv

@@ -8,7 +8,6 @@
 #include <algorithm>
 #include <cstring>
 #include <new>
-#include <queue>
 
 #include "fcp_internal.h"
 
@@ -16,38 +15,72 @@ namespace {
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 // Persistent grid size = SM count of the current device (148 on B200; also the value used when
-// no device is visible, e.g. when a schedule is built on a CPU-only box).
+// no device is visible, e.g. when a schedule is built on a CPU-only box).  Cached per device:
+// the query costs more than the rest of a small schedule.
 int32_t grid_ctas() {
-  int dev = 0, n = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess ||
-      cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
+  static int cached_dev = -2, cached_n = 148;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
     cudaGetLastError();
-    return 148;
+    dev = -1;
   }
+  if (dev == cached_dev) return cached_n;
+  int n = 0;
+  if (dev < 0 || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
+    cudaGetLastError();
+    n = 148;
+  }
+  cached_dev = dev;
+  cached_n = n;
   return n;
 }
 
+// Stable sort by descending integer key (counting sort: the keys are tile / iteration counts).
+template <typename Item, typename Key>
+void stable_sort_desc(std::vector<Item>& v, Key key) {
+  int64_t mx = 0;
+  for (const Item& x : v) mx = std::max<int64_t>(mx, key(x));
+  std::vector<int32_t> pos((size_t)mx + 2, 0);
+  for (const Item& x : v) ++pos[(size_t)(mx - key(x)) + 1];
+  for (size_t i = 1; i < pos.size(); ++i) pos[i] += pos[i - 1];
+  std::vector<Item> out(v.size());
+  for (const Item& x : v) out[pos[(size_t)(mx - key(x))]++] = x;
+  v.swap(out);
+}
+
 // Greedy longest-processing-time assignment of items (already sorted by descending cost) to
-// n_cta persistent CTAs; `items` is permuted so that every CTA's list is contiguous and
-// cta_off[c] .. cta_off[c+1] delimits it.  Deterministic: ties go to the lowest CTA index.
+// n_cta persistent CTAs; `items` is permuted so that every CTA's list is contiguous (in the
+// order the items were assigned) and cta_off[c] .. cta_off[c+1] delimits it.  Deterministic:
+// the next item goes to the least loaded CTA, ties to the lowest CTA index.  Binary min-heap of
+// (load, cta) with replace-top; the permutation is a counting scatter.
 template <typename Item, typename Cost>
 void assign_lpt(std::vector<Item>& items, int32_t n_cta, Cost cost, std::vector<int32_t>& cta_off) {
   typedef std::pair<int64_t, int32_t> Load;      // (load, cta)
-  std::priority_queue<Load, std::vector<Load>, std::greater<Load>> heap;
-  for (int32_t c = 0; c < n_cta; ++c) heap.push(Load(0, c));
-  std::vector<std::vector<Item>> bins(n_cta);
-  for (const Item& it : items) {
-    Load l = heap.top();
-    heap.pop();
-    bins[l.second].push_back(it);
-    heap.push(Load(l.first + cost(it), l.second));
+  std::vector<Load> heap((size_t)n_cta);
+  for (int32_t c = 0; c < n_cta; ++c) heap[c] = Load(0, c);     // ascending = a valid heap
+  std::vector<int32_t> owner(items.size());
+  cta_off.assign((size_t)n_cta + 1, 0);
+  for (size_t i = 0; i < items.size(); ++i) {
+    owner[i] = heap[0].second;
+    ++cta_off[(size_t)owner[i] + 1];
+    Load top(heap[0].first + cost(items[i]), heap[0].second);
+    size_t h = 0;                                 // sift the updated top down
+    for (;;) {
+      size_t l = 2 * h + 1, r = l + 1, m = h;
+      Load best = top;
+      if (l < heap.size() && heap[l] < best) { best = heap[l]; m = l; }
+      if (r < heap.size() && heap[r] < best) { best = heap[r]; m = r; }
+      if (m == h) break;
+      heap[h] = heap[m];
+      h = m;
+    }
+    heap[h] = top;
   }
-  cta_off.assign(n_cta + 1, 0);
-  size_t k = 0;
-  for (int32_t c = 0; c < n_cta; ++c) {
-    for (const Item& it : bins[c]) items[k++] = it;
-    cta_off[c + 1] = (int32_t)k;
-  }
+  for (int32_t c = 0; c < n_cta; ++c) cta_off[(size_t)c + 1] += cta_off[c];
+  std::vector<int32_t> pos(cta_off.begin(), cta_off.end() - 1);
+  std::vector<Item> out(items.size());
+  for (size_t i = 0; i < items.size(); ++i) out[(size_t)pos[owner[i]]++] = items[i];
+  items.swap(out);
 }
 }
 
@@ -118,8 +151,7 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
       s->tile_meta.push_back(std::min(FCP_BQ, len - r0));
     }
   }
-  std::stable_sort(s->fwd.begin(), s->fwd.end(),
-                   [](const FwdItem& x, const FwdItem& y) { return x.n_kv_tiles > y.n_kv_tiles; });
+  stable_sort_desc(s->fwd, [](const FwdItem& x) { return (int64_t)x.n_kv_tiles; });
   s->n_cta = grid_ctas();
   // cost in KV-tile steps; +1 for the per-item Q load and epilogue
   assign_lpt(s->fwd, s->n_cta, [](const FwdItem& x) { return (int64_t)x.n_kv_tiles + 1; },
@@ -161,8 +193,7 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
       }
     }
   }
-  std::stable_sort(s->bwd.begin(), s->bwd.end(),
-                   [](const BwdItem& x, const BwdItem& y) { return x.n_iters > y.n_iters; });
+  stable_sort_desc(s->bwd, [](const BwdItem& x) { return (int64_t)x.n_iters; });
   // cost in inner iterations; +2 for the per-item K/V load and the dK/dV epilogue
   assign_lpt(s->bwd, s->n_cta, [](const BwdItem& x) { return (int64_t)x.n_iters + 2; },
              s->bwd_cta_off);

@@ -442,6 +442,39 @@ def test_sixteen_byte_aligned_outputs(fcp, torch):
         sched.attn_fwd(q, kg, vg, scale, o=o8)
 
 
+@pytest.mark.parametrize("name", ["8b", "short"])
+def test_run_to_run_determinism(fcp, torch, name):
+    """Race detector: the kernels are deep asynchronous pipelines (TMA, tcgen05, mbarriers, TMEM
+    operands overwritten in place).  Everything except dq is computed in a fixed order, so o, lse,
+    dk, dv must be bit-identical from run to run on the bench shapes; dq is summed by L2
+    reductions whose order varies — it may move by an ulp of its bf16 rounding, not more."""
+    cfg = fcp_inputs.CONFIGS[name]
+    d = fcp_inputs.doc_lengths(name, 0)
+    scale = 1.0 / math.sqrt(cfg.D)
+    plan = fcp.Plan(d, cfg.N)
+    gen = torch.Generator(device="cuda").manual_seed(7)
+    K = torch.randn((cfg.C, cfg.Hkv, cfg.D), device="cuda", generator=gen).bfloat16()
+    V = torch.randn((cfg.C, cfg.Hkv, cfg.D), device="cuda", generator=gen).bfloat16()
+    r = cfg.N - 1
+    n_q = plan.rank_stats(r)["n_q"]
+    q = torch.randn((n_q, cfg.Hq, cfg.D), device="cuda", generator=gen).bfloat16()
+    do = torch.randn((n_q, cfg.Hq, cfg.D), device="cuda", generator=gen).bfloat16()
+    sched = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload("cuda")
+    kg, vg, _ = plan.kv_gather(r, K, V)
+    ref = None
+    for it in range(12):
+        o, lse = sched.attn_fwd(q, kg, vg, scale)
+        dq, dk, dv = sched.attn_bwd(q, kg, vg, o, lse, do, scale)
+        torch.cuda.synchronize()
+        cur = [t.clone() for t in (o, lse, dk, dv)]
+        if ref is None:
+            ref, dq_ref = cur, dq.float().clone()
+            continue
+        for a, b, nm in zip(cur, ref, ("o", "lse", "dk", "dv")):
+            assert torch.equal(a, b), "%s differs in repetition %d" % (nm, it)
+        assert float((dq.float() - dq_ref).abs().max()) <= 2e-3 * max(1.0, float(dq_ref.abs().max()))
+
+
 def test_missing_library_fails_loudly(fcp, monkeypatch):
     import paper_2606_08476_b200.binding as B
     monkeypatch.setattr(B, "_LIB", None)

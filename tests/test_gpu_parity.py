@@ -207,6 +207,29 @@ def test_8b_config_one_gqa_group(fcp, torch, dkv_f32):
     U.check("dv", U.to_f64(g["dv"][:, hk:hk + 1]), w["dv"], bf16_sum=not dkv_f32)
 
 
+@pytest.mark.parametrize("name,r,hk", [("short", 7, 2), ("longtail", 3, 6), ("70b", 5, 1)])
+def test_full_size_configs_one_gqa_group(fcp, torch, name, r, hk):
+    """The other BASELINE.json configs at full size, in the launch configuration bench.py times
+    (all heads, tensors drawn on the device as bench.py does): the oracle checks every row of one
+    GQA group of one virtual rank, forward and backward (heads are independent units, SURVEY
+    8(d)).  longtail and 70b put Per-Doc shards with 70K-key prefixes and G = 8 on the kernels."""
+    cfg = fcp_inputs.CONFIGS[name]
+    d = fcp_inputs.doc_lengths(name, 0)
+    scale = 1.0 / math.sqrt(cfg.D)
+    Q, K, V, dO = fcp_inputs.make_tensors(cfg.C, cfg.Hq, cfg.Hkv, cfg.D, 0, device="cuda")
+    plan = fcp.Plan(d, cfg.N)
+    G = cfg.Hq // cfg.Hkv
+    g = U.run_rank_gpu(fcp, plan, r, Q, K, V, dO, scale)
+    hq = slice(hk * G, (hk + 1) * G)
+    w = U.run_rank_oracle(d, cfg.N, r, U.to_f64(Q[:, hq]), U.to_f64(K[:, hk:hk + 1]),
+                          U.to_f64(V[:, hk:hk + 1]), U.to_f64(dO[:, hq]), scale)
+    U.check("o", U.to_f64(g["o"][:, hq]), w["o"])
+    U.check_lse("lse", U.to_f64(g["lse"][hq]), w["lse"])
+    U.check("dq", U.to_f64(g["dq"][:, hq]), w["dq"])
+    U.check("dk", U.to_f64(g["dk"][:, hk:hk + 1]), w["dk"], bf16_sum=True)
+    U.check("dv", U.to_f64(g["dv"][:, hk:hk + 1]), w["dv"], bf16_sum=True)
+
+
 def test_kv_pieces_and_merge(fcp, torch):
     """Split every shard's keys at c into two pieces (second piece: negative q_pos_off, rows that
     see no key), run each piece through fcp_attn_fwd, combine with fcp_merge; backward through

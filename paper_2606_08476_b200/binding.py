@@ -307,9 +307,18 @@ class Sched:
         _check(_lib().fcp_sched_workspace_size(self._h, C.byref(n)), "fcp_sched_workspace_size")
         return n.value
 
-    def upload(self, device="cuda", stream=None):
+    def upload(self, device="cuda", stream=None, workspace=None):
+        """Copy the item lists into the device workspace (allocated here unless the caller passes
+        a uint8 tensor of at least workspace_size() bytes that it keeps alive and reuses; the
+        caller then orders the copy stream against the kernels that still read the old lists)."""
         import torch
-        self.workspace = torch.empty(self.workspace_size(), dtype=torch.uint8, device=device)
+        if workspace is None:
+            workspace = torch.empty(self.workspace_size(), dtype=torch.uint8, device=device)
+        elif workspace.dtype != torch.uint8 or workspace.numel() < self.workspace_size() or \
+                not workspace.is_cuda or not workspace.is_contiguous():
+            raise ValueError("workspace must be a contiguous cuda uint8 tensor of >= %d bytes"
+                             % self.workspace_size())
+        self.workspace = workspace
         _check(_lib().fcp_sched_upload(self._h, self.workspace.data_ptr(), _stream_ptr(stream)),
                "fcp_sched_upload")
         return self

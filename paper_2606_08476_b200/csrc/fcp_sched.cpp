@@ -51,30 +51,42 @@ void stable_sort_desc(std::vector<Item>& v, Key key) {
 // Greedy longest-processing-time assignment of items (already sorted by descending cost) to
 // n_cta persistent CTAs; `items` is permuted so that every CTA's list is contiguous (in the
 // order the items were assigned) and cta_off[c] .. cta_off[c+1] delimits it.  Deterministic:
-// the next item goes to the least loaded CTA, ties to the lowest CTA index.  Binary min-heap of
-// (load, cta) with replace-top; the permutation is a counting scatter.
+// the next item goes to the least loaded CTA, ties to the lowest CTA index.  Costs are small
+// positive integers, so the priority queue is a bucket queue: bucket[l] = bit set of the CTAs
+// with load l.  The least load never decreases (every cost is >= 1) and never exceeds
+// avg + max cost, so one pointer walks the buckets once; taking the next CTA is a
+// count-trailing-zeros.  (A binary heap of (load, cta) pairs gives the same lists at ~90 ns
+// per item: 2/3 of the build time of a schedule of short documents.)  The permutation is a
+// counting scatter.
 template <typename Item, typename Cost>
 void assign_lpt(std::vector<Item>& items, int32_t n_cta, Cost cost, std::vector<int32_t>& cta_off) {
-  typedef std::pair<int64_t, int32_t> Load;      // (load, cta)
-  std::vector<Load> heap((size_t)n_cta);
-  for (int32_t c = 0; c < n_cta; ++c) heap[c] = Load(0, c);     // ascending = a valid heap
+  const size_t words = ((size_t)n_cta + 63) / 64;
+  int64_t total = 0, mx = 1;
+  for (const Item& x : items) {
+    const int64_t c = cost(x);
+    total += c;
+    mx = std::max(mx, c);
+  }
+  const size_t n_buckets = (size_t)(total / n_cta + mx + 2);
+  std::vector<uint64_t> bucket(n_buckets * words, 0);
+  for (int32_t c = 0; c < n_cta; ++c) bucket[(size_t)c / 64] |= 1ull << (c % 64);   // all at load 0
   std::vector<int32_t> owner(items.size());
   cta_off.assign((size_t)n_cta + 1, 0);
+  size_t lo = 0;                                  // least load with a CTA in its bucket
   for (size_t i = 0; i < items.size(); ++i) {
-    owner[i] = heap[0].second;
-    ++cta_off[(size_t)owner[i] + 1];
-    Load top(heap[0].first + cost(items[i]), heap[0].second);
-    size_t h = 0;                                 // sift the updated top down
+    size_t w = 0;
     for (;;) {
-      size_t l = 2 * h + 1, r = l + 1, m = h;
-      Load best = top;
-      if (l < heap.size() && heap[l] < best) { best = heap[l]; m = l; }
-      if (r < heap.size() && heap[r] < best) { best = heap[r]; m = r; }
-      if (m == h) break;
-      heap[h] = heap[m];
-      h = m;
+      for (w = 0; w < words && bucket[lo * words + w] == 0; ++w) {}
+      if (w < words) break;
+      ++lo;
     }
-    heap[h] = top;
+    uint64_t& word = bucket[lo * words + w];
+    const int32_t c = (int32_t)(w * 64 + (size_t)__builtin_ctzll(word));
+    word &= word - 1;
+    owner[i] = c;
+    ++cta_off[(size_t)c + 1];
+    const size_t nl = lo + (size_t)cost(items[i]);
+    bucket[nl * words + (size_t)c / 64] |= 1ull << (c % 64);
   }
   for (int32_t c = 0; c < n_cta; ++c) cta_off[(size_t)c + 1] += cta_off[c];
   std::vector<int32_t> pos(cta_off.begin(), cta_off.end() - 1);
@@ -84,10 +96,11 @@ void assign_lpt(std::vector<Item>& items, int32_t n_cta, Cost cost, std::vector<
 }
 }
 
-extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
-                                const int32_t* shard_seg, int32_t n_shards,
-                                const int32_t* cu_seqlens_k, int32_t n_segs, int32_t n_q_heads,
-                                int32_t n_kv_heads, int32_t head_dim, fcp_sched** out) {
+// n_cta: size of the persistent grid
+static int sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
+                        const int32_t* shard_seg, int32_t n_shards, const int32_t* cu_seqlens_k,
+                        int32_t n_segs, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                        int32_t n_cta, fcp_sched** out) {
   if (!cu_seqlens_q || !q_pos_off || !shard_seg || !cu_seqlens_k || !out || n_shards < 0 ||
       n_segs < 0 || n_q_heads < 1 || n_kv_heads < 1)
     return FCP_INVALID_ARG;
@@ -114,6 +127,7 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
   // ---- forward items ----
   const int packs = s->G / s->NQ;
   s->shard_pad0.resize(n_shards);
+  s->fwd.reserve((size_t)((s->n_q + FCP_TQ - 1) / FCP_TQ + n_shards) * s->Hkv * packs);
   int64_t pad = 0;
   for (int i = 0; i < n_shards; ++i) {
     const int32_t a = s->cu_q[i], len = s->cu_q[i + 1] - a, p = s->q_pos_off[i];
@@ -121,9 +135,14 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
     const int32_t kv0 = s->cu_k[g], kvl = s->cu_k[g + 1] - kv0;
     s->shard_pad0[i] = (int32_t)pad;
     pad += (int64_t)(len + FCP_BQ - 1) / FCP_BQ * FCP_BQ;
-    for (int32_t t = 0; t < len; ++t) {          // exact unmasked-pair count (statistic)
-      const int64_t vis = std::min<int64_t>(kvl, (int64_t)p + t + 1);
-      if (vis > 0) s->useful_pairs += (uint64_t)vis;
+    // exact unmasked-pair count (statistic): sum over rows t of clamp(p + t + 1, 0, kvl) --
+    // zero up to row t_lo, p + t + 1 up to row t_hi, kvl from there on
+    if (kvl > 0 && len > 0) {
+      const int64_t a = (int64_t)p + 1;
+      const int64_t t_lo = std::min<int64_t>(len, std::max<int64_t>(0, 1 - a));
+      const int64_t t_hi = std::min<int64_t>(len, std::max<int64_t>(t_lo, (int64_t)kvl - a));
+      const int64_t m = t_hi - t_lo;
+      s->useful_pairs += (uint64_t)(m * a + (t_lo + t_hi - 1) * m / 2 + (len - t_hi) * (int64_t)kvl);
     }
     for (int32_t r0 = 0; r0 < len; r0 += FCP_TQ) {
       FwdItem it;
@@ -152,7 +171,7 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
     }
   }
   stable_sort_desc(s->fwd, [](const FwdItem& x) { return (int64_t)x.n_kv_tiles; });
-  s->n_cta = grid_ctas();
+  s->n_cta = n_cta;
   // cost in KV-tile steps; +1 for the per-item Q load and epilogue
   assign_lpt(s->fwd, s->n_cta, [](const FwdItem& x) { return (int64_t)x.n_kv_tiles + 1; },
              s->fwd_cta_off);
@@ -227,6 +246,23 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
   return FCP_OK;
 }
 
+extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
+                                const int32_t* shard_seg, int32_t n_shards,
+                                const int32_t* cu_seqlens_k, int32_t n_segs, int32_t n_q_heads,
+                                int32_t n_kv_heads, int32_t head_dim, fcp_sched** out) {
+  return sched_create(cu_seqlens_q, q_pos_off, shard_seg, n_shards, cu_seqlens_k, n_segs,
+                      n_q_heads, n_kv_heads, head_dim, grid_ctas(), out);
+}
+
+static int sched_from_plan(const fcp_plan* plan, int32_t rank, int32_t piece, int32_t n_q_heads,
+                           int32_t n_kv_heads, int32_t head_dim, int32_t n_cta, fcp_sched** out) {
+  RankView v;
+  fcp_build_rank_view(*plan, rank, v, piece);
+  return sched_create(v.cu_q.data(), v.q_pos_off.data(), v.shard_seg.data(),
+                      (int32_t)v.q_pos_off.size(), v.cu_k.data(), (int32_t)v.kv_len.size(),
+                      n_q_heads, n_kv_heads, head_dim, n_cta, out);
+}
+
 extern "C" int fcp_sched_from_plan(const fcp_plan* plan, int32_t rank, int32_t n_q_heads,
                                    int32_t n_kv_heads, int32_t head_dim, fcp_sched** out) {
   return fcp_sched_from_plan_piece(plan, rank, FCP_PIECE_FULL, n_q_heads, n_kv_heads, head_dim, out);
@@ -238,11 +274,7 @@ extern "C" int fcp_sched_from_plan_piece(const fcp_plan* plan, int32_t rank, int
   if (!plan || !out || rank < 0 || rank >= plan->n_ranks ||
       (piece != FCP_PIECE_FULL && piece != FCP_PIECE_LOCAL && piece != FCP_PIECE_PREFIX))
     return FCP_INVALID_ARG;
-  RankView v;
-  fcp_build_rank_view(*plan, rank, v, piece);
-  return fcp_sched_create(v.cu_q.data(), v.q_pos_off.data(), v.shard_seg.data(),
-                          (int32_t)v.q_pos_off.size(), v.cu_k.data(), (int32_t)v.kv_len.size(),
-                          n_q_heads, n_kv_heads, head_dim, out);
+  return sched_from_plan(plan, rank, piece, n_q_heads, n_kv_heads, head_dim, grid_ctas(), out);
 }
 
 extern "C" void fcp_sched_destroy(fcp_sched* sched) { delete sched; }

@@ -611,6 +611,8 @@ def run_fcp(args):
                          "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",
                          "frac": bwd_tf / peaks["bf16_sustained"], "traffic": traffic,
                          "peak_source": peaks["source"] + " cuBLAS bf16, sustained",
+                         "frac_of_burst_peak": bwd_tf / peaks["bf16"],
+                         "burst_peak": peaks["bf16"],
                          "frac_of_nominal_2250": bwd_tf / NOMINAL_BF16_TFLOPS},
             "kernels": {
                 "attn_fwd": {"tflops": fwd_tf, "frac_measured": fwd_tf / peaks["bf16_sustained"],

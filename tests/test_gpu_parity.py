@@ -498,6 +498,35 @@ def test_run_to_run_determinism(fcp, torch, name):
         assert float((dq.float() - dq_ref).abs().max()) <= 2e-3 * max(1.0, float(dq_ref.abs().max()))
 
 
+def test_caller_owned_workspace_on_a_copy_stream(fcp, torch):
+    """Sched.upload(workspace=, stream=): the caller keeps one workspace alive across steps and
+    sends the lists up on its own copy stream (what bench.py does); same bits as the default
+    path, and a workspace that is too small is refused."""
+    d, N, Hq, Hkv, D = [700, 300, 24], 2, 4, 2, 128
+    scale = 1.0 / math.sqrt(D)
+    Q, K, V, dO = (t.cuda() for t in fcp_inputs.make_tensors(sum(d), Hq, Hkv, D, 3))
+    plan = fcp.Plan(d, N)
+    ref = U.run_rank_gpu(fcp, plan, 1, Q, K, V, dO, scale)
+    sched = plan.sched(1, Hq, Hkv, D)
+    with pytest.raises(ValueError):
+        sched.upload("cuda", workspace=torch.empty(sched.workspace_size() - 1, dtype=torch.uint8,
+                                                   device="cuda"))
+    ws = torch.full((sched.workspace_size() + 4096,), 0xA5, dtype=torch.uint8, device="cuda")
+    side = torch.cuda.Stream()
+    ready = torch.cuda.Event()
+    for step in range(2):                    # second round: the workspace holds the old lists and dq
+        side.wait_stream(torch.cuda.current_stream())
+        sched = plan.sched(1, Hq, Hkv, D).upload("cuda", stream=side, workspace=ws)
+        ready.record(side)
+        torch.cuda.current_stream().wait_event(ready)
+        o, lse = sched.attn_fwd(ref["q"], ref["k"], ref["v"], scale)
+        dq, dk, dv = sched.attn_bwd(ref["q"], ref["k"], ref["v"], o, lse, ref["do"], scale)
+        torch.cuda.synchronize()
+        for name, got in (("o", o), ("lse", lse), ("dq", dq), ("dk", dk), ("dv", dv)):
+            assert torch.equal(got, ref[name]), (step, name)
+    assert bool((ws[sched.workspace_size():] == 0xA5).all())
+
+
 def test_missing_library_fails_loudly(fcp, monkeypatch):
     import paper_2606_08476_b200.binding as B
     monkeypatch.setattr(B, "_LIB", None)

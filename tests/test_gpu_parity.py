@@ -500,8 +500,8 @@ def test_run_to_run_determinism(fcp, torch, name):
 
 def test_caller_owned_workspace_on_a_copy_stream(fcp, torch):
     """Sched.upload(workspace=, stream=): the caller keeps one workspace alive across steps and
-    sends the lists up on its own copy stream (what bench.py does); same bits as the default
-    path, and a workspace that is too small is refused."""
+    sends the lists up on its own copy stream (what bench.py does); same results as the default
+    path (same bits where the path is deterministic), and a workspace that is too small is refused."""
     d, N, Hq, Hkv, D = [700, 300, 24], 2, 4, 2, 128
     scale = 1.0 / math.sqrt(D)
     Q, K, V, dO = (t.cuda() for t in fcp_inputs.make_tensors(sum(d), Hq, Hkv, D, 3))
@@ -522,8 +522,10 @@ def test_caller_owned_workspace_on_a_copy_stream(fcp, torch):
         o, lse = sched.attn_fwd(ref["q"], ref["k"], ref["v"], scale)
         dq, dk, dv = sched.attn_bwd(ref["q"], ref["k"], ref["v"], o, lse, ref["do"], scale)
         torch.cuda.synchronize()
-        for name, got in (("o", o), ("lse", lse), ("dq", dq), ("dk", dk), ("dv", dv)):
+        for name, got in (("o", o), ("lse", lse), ("dk", dk), ("dv", dv)):
             assert torch.equal(got, ref[name]), (step, name)
+        # dq is a sum of fp32 reductions whose order is not fixed (test_run_to_run_determinism)
+        torch.testing.assert_close(dq.float(), ref["dq"].float(), rtol=2.0 ** -6, atol=1e-3)
     assert bool((ws[sched.workspace_size():] == 0xA5).all())
 
 

@@ -217,6 +217,27 @@ typedef struct {
 } fcp_sched_info;
 int  fcp_sched_get_info(const fcp_sched* sched, fcp_sched_info* out);
 
+/* Read-back of the host work lists as int32 words (what fcp_sched_upload sends to the device;
+ * for tests and tools).  `which`:
+ *   FCP_LIST_FWD_ITEMS  8 words per item, grouped by CTA in processing order:
+ *                       q_row0, q_rows, kv_row0, kv_len, q_pos0, n_kv_tiles, head0, kv_head
+ *                       (one 128-row q tile of one shard x one pack of 1 or 2 query heads of one
+ *                       kv head; KV tiles [0, n_kv_tiles) of 128 rows are visited, later tiles
+ *                       are fully masked)
+ *   FCP_LIST_BWD_ITEMS  8 words per item: kv_row0, kv_rows, kv_pos0, kv_head, sub_begin,
+ *                       sub_end, n_iters, 0   (one 128-row KV tile of one segment x one kv head)
+ *   FCP_LIST_BWD_SUBS   4 words per entry: q_row0, q_pos0, q_rows, pad_row0 (a shard seen by a
+ *                       KV tile, from the first 64-row q tile that sees it to the shard's end)
+ *   FCP_LIST_FWD_CTA / FCP_LIST_BWD_CTA   n_cta + 1 offsets: CTA c owns items [off[c], off[c+1])
+ * Items are sorted by descending cost (n_kv_tiles + 1, n_iters + 2; stable in enumeration order:
+ * shards, q tiles, kv heads, packs / segments, KV tiles, kv heads) and handed one by one to the
+ * least loaded CTA, ties to the lowest CTA index.  Writes min(cap_words, n) words and the total
+ * n to *n_words. */
+enum { FCP_LIST_FWD_ITEMS = 0, FCP_LIST_BWD_ITEMS = 1, FCP_LIST_BWD_SUBS = 2, FCP_LIST_FWD_CTA = 3,
+       FCP_LIST_BWD_CTA = 4 };
+int  fcp_sched_get_list(const fcp_sched* sched, int32_t which, int32_t* out, int64_t cap_words,
+                        int64_t* n_words);
+
 /* ------------------------------------------------------------------------------------------
  * 4. Document-masked causal attention, forward and backward.
  *      forward : o = softmax(scale q K^T + mask) V, lse = log sum exp   (per shard, per head)

@@ -15,7 +15,7 @@ EXPORTS = [
     "fcp_kv_gather", "fcp_kv_scatter_add", "fcp_sched_create", "fcp_sched_from_plan", "fcp_sched_destroy",
     "fcp_sched_workspace_size", "fcp_sched_upload", "fcp_sched_get_info", "fcp_attn_fwd",
     "fcp_attn_bwd", "fcp_merge", "fcp_plan_piece_stats", "fcp_piece_layout", "fcp_kv_gather_piece",
-    "fcp_kv_scatter_add_piece", "fcp_sched_from_plan_piece",
+    "fcp_kv_scatter_add_piece", "fcp_sched_from_plan_piece", "fcp_sched_get_list",
 ]
 
 STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC, STRATEGY_PER_SEQ = 0, 1, 2, 3
@@ -126,6 +126,8 @@ def _lib():
         lib.fcp_sched_workspace_size.argtypes = [C.c_void_p, C.POINTER(C.c_size_t)]
         lib.fcp_sched_upload.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.fcp_sched_get_info.argtypes = [C.c_void_p, C.POINTER(_SchedInfo)]
+        lib.fcp_sched_get_list.argtypes = [C.c_void_p, C.c_int32, _I32P, C.c_int64,
+                                           C.POINTER(C.c_int64)]
         lib.fcp_attn_fwd.argtypes = [C.POINTER(_AttnArgs)]
         lib.fcp_attn_bwd.argtypes = [C.POINTER(_AttnArgs), C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p]
@@ -301,6 +303,22 @@ class Sched:
         s = _SchedInfo()
         _check(_lib().fcp_sched_get_info(self._h, C.byref(s)), "fcp_sched_get_info")
         return _struct_dict(s)
+
+    def lists(self):
+        """Host work lists (fcp_sched_get_list) as int32 arrays: fwd [n,8], bwd [n,8], sub [n,4],
+        fwd_cta / bwd_cta [n_cta+1]; field order in include/fcp.h."""
+        out = {}
+        for name, which, width in (("fwd", 0, 8), ("bwd", 1, 8), ("sub", 2, 4), ("fwd_cta", 3, 1),
+                                   ("bwd_cta", 4, 1)):
+            n = C.c_int64()
+            _check(_lib().fcp_sched_get_list(self._h, which, None, 0, C.byref(n)),
+                   "fcp_sched_get_list")
+            a = np.zeros(max(n.value, 1), dtype=np.int32)
+            _check(_lib().fcp_sched_get_list(self._h, which, _p(a), n.value, C.byref(n)),
+                   "fcp_sched_get_list")
+            a = a[:n.value]
+            out[name] = a.reshape(-1, width) if width > 1 else a
+        return out
 
     def workspace_size(self):
         n = C.c_size_t()

@@ -297,3 +297,23 @@ extern "C" int fcp_sched_get_info(const fcp_sched* sched, fcp_sched_info* out) {
   out->n_q_pad = sched->n_q_pad;
   return FCP_OK;
 }
+
+extern "C" int fcp_sched_get_list(const fcp_sched* sched, int32_t which, int32_t* out,
+                                  int64_t cap_words, int64_t* n_words) {
+  if (!sched || !n_words || cap_words < 0 || (cap_words > 0 && !out)) return FCP_INVALID_ARG;
+  static_assert(sizeof(FwdItem) == 32 && sizeof(BwdItem) == 32 && sizeof(BwdSub) == 16, "layout");
+  const void* src = nullptr;
+  int64_t n = 0;
+  switch (which) {
+    case FCP_LIST_FWD_ITEMS: src = sched->fwd.data();         n = (int64_t)sched->fwd.size() * 8; break;
+    case FCP_LIST_BWD_ITEMS: src = sched->bwd.data();         n = (int64_t)sched->bwd.size() * 8; break;
+    case FCP_LIST_BWD_SUBS:  src = sched->bwd_sub.data();     n = (int64_t)sched->bwd_sub.size() * 4; break;
+    case FCP_LIST_FWD_CTA:   src = sched->fwd_cta_off.data(); n = (int64_t)sched->fwd_cta_off.size(); break;
+    case FCP_LIST_BWD_CTA:   src = sched->bwd_cta_off.data(); n = (int64_t)sched->bwd_cta_off.size(); break;
+    default: return FCP_INVALID_ARG;
+  }
+  *n_words = n;
+  const int64_t m = std::min(n, cap_words);
+  if (m > 0) std::memcpy(out, src, (size_t)m * sizeof(int32_t));
+  return FCP_OK;
+}

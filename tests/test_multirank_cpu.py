@@ -74,3 +74,89 @@ def test_single_process_is_identity():
     assert bench.over_ranks(3.5, "max") == 3.5
     v, ms = bench.job_throughput(2e12, 1000.0)
     assert ms == 1000.0 and v == pytest.approx(2.0)
+
+
+# ------------------------------------------------------------------------------------------
+# KV exchange of a real CP group (paper_2606_08476_b200/exchange.py) on gloo ranks
+# ------------------------------------------------------------------------------------------
+_XCASES = {
+    2: ([700, 90, 300, 190], 0),          # Per-Doc pair + whole documents
+    4: ([2048, 37, 1, 600, 130, 256], 0),  # long document split over all ranks, 1-token document
+}
+
+
+def _xchg_grads(n_rows, Hkv, D, r):
+    import torch
+    g = torch.Generator().manual_seed(1000 + r)
+    return (torch.randn((n_rows, Hkv, D), generator=g), torch.randn((n_rows, Hkv, D), generator=g))
+
+
+def _xchg_worker(rank, world, port, out):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    import fcp_inputs
+    import paper_2606_08476_b200 as fcp
+    from paper_2606_08476_b200.exchange import KVExchange
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        d, strategy = _XCASES[world]
+        Hkv, D = 2, 64
+        _, K, V, _ = fcp_inputs.make_tensors(sum(d), 2, Hkv, D, 3)
+        plan = fcp.Plan(d, world, strategy=strategy)
+        x = KVExchange(plan, rank)
+        lay = plan.rank_layout(rank)
+        qi = torch.from_numpy(lay["q_token_index"].astype(np.int64))
+        k, v = x.gather(K[qi].contiguous(), V[qi].contiguous())      # this rank holds only its rows
+        dk_r, dv_r = _xchg_grads(x.n_kv, Hkv, D, rank)
+        dk_l, dv_l = x.scatter_add(dk_r, dv_r)
+        out.put((rank, k.view(torch.int16).numpy(), v.view(torch.int16).numpy(), dk_l.numpy(),
+                 dv_l.numpy(), x.remote_tokens, plan.rank_stats(rank)["remote_tokens"]))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 4])
+def test_kv_exchange_matches_oracle_gather_and_scatter(world):
+    """Each gloo rank starts with its own K, V rows only; after the all-to-all-v it holds exactly
+    the rows the ORACLE's gather index names (bit-exact), having received exactly the planner's
+    remote-token count; the way back sums every rank's dk, dv rows onto their owners as the
+    oracle's token-by-token scatter does."""
+    import numpy as np
+    import torch
+    import torch.multiprocessing as mp
+    import fcp_inputs
+    from oracle import kvselect as KV
+    from oracle import planner as P
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_xchg_worker, args=(r, world, port, out)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((out.get(timeout=240) for _ in procs), key=lambda t: t[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    d, strategy = _XCASES[world]
+    Hkv, D = 2, 64
+    _, K, V, _ = fcp_inputs.make_tensors(sum(d), 2, Hkv, D, 3)
+    Ki, Vi = K.view(torch.int16).numpy(), V.view(torch.int16).numpy()
+    pl = P.plan(d, world, 1_050_000, strategy)
+    kst = KV.kv_stats(pl)
+    dK = np.zeros((sum(d), Hkv, D))
+    dV = np.zeros_like(dK)
+    for r in range(world):                                  # rank order, one add per element and rank
+        gi = KV.gather_index(pl, r)
+        gk, gv = _xchg_grads(len(gi), Hkv, D, r)
+        dK[gi] += gk.double().numpy()
+        dV[gi] += gv.double().numpy()
+    for r, k, v, dk_l, dv_l, remote, remote_plan in res:
+        gi = KV.gather_index(pl, r)
+        assert np.array_equal(k, Ki[gi]) and np.array_equal(v, Vi[gi])
+        assert remote == remote_plan == kst.remote[r]
+        qi = KV.q_token_index(pl, r)
+        assert np.abs(dk_l - dK[qi]).max() < 1e-5 and np.abs(dv_l - dV[qi]).max() < 1e-5
+    assert sum(t[5] for t in res) > 0                       # the case really moves rows

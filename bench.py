@@ -605,7 +605,7 @@ def run_fcp(args):
                        "l2": "inputs larger than L2 (per-rank q,o,dO,dq + fp32 dq scratch "
                              "= %.0f MiB vs 126 MB L2)" % (
                                  cfg.C // cfg.N * cfg.Hq * cfg.D * (4 * 2 + 4) / 2 ** 20),
-                       "step": "plan + per virtual rank: schedule upload, KV gather, fwd, bwd"},
+                       "step": "plan + per virtual rank: schedule build + upload (copy stream), KV gather, fwd, bwd"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": 5 * cfg.N * args.steps,
             "roofline": {"bound": "tensor", "kernel": "fcp_attn_bwd_main", "achieved": bwd_tf,
                          "peak": peaks["bf16_sustained"], "unit": "TFLOP/s",

@@ -9,7 +9,12 @@
  *
  * General rules
  *  - Every function returns an int: FCP_OK (0) or a negative fcp_status.  Nothing throws or
- *    aborts across this boundary and there is no global mutable state.
+ *    aborts across this boundary (host allocation failures come back as FCP_NO_MEMORY).  The
+ *    library keeps no mutable state of its own besides the objects it hands out: the only
+ *    process-wide data are write-once caches of immutable facts (the SM count per device, the
+ *    address of the driver's tensor-map encoder), published with atomics, so every entry point
+ *    may be called from several threads and for several devices.  Objects are not internally
+ *    synchronised: do not destroy one while another thread uses it.
  *  - "host" pointers are ordinary CPU memory; "device" pointers are CUDA device memory of the
  *    current device.  The library owns only the opaque host objects it creates (fcp_plan,
  *    fcp_sched).  It never allocates, frees or synchronises device memory: inputs, outputs
@@ -36,7 +41,8 @@ typedef enum {
   FCP_UNSUPPORTED = -2,      /* D not in {64,128}, Hq % Hkv != 0, unknown dtype/strategy */
   FCP_BUFFER_TOO_SMALL = -3, /* required element count is written to *n_out */
   FCP_CUDA = -4,             /* a CUDA runtime/driver call or kernel launch failed */
-  FCP_MISALIGNED = -5        /* a device pointer or row pitch is not 16-byte aligned */
+  FCP_MISALIGNED = -5,       /* a device pointer or row pitch is not 16-byte aligned */
+  FCP_NO_MEMORY = -6         /* a host allocation failed (std::bad_alloc is caught at the boundary) */
 } fcp_status;
 
 const char* fcp_strerror(int status);
@@ -59,7 +65,15 @@ typedef struct {
   int64_t imbalance_ppm;   /* target R = max/avg workload times 1e6; >= 1000000;
                               0 selects the default 1050000 */
   int32_t strategy;        /* FCP_STRATEGY_* */
-  int32_t reserved;        /* must be 0 */
+  int32_t align_tokens;    /* 0 or 1: Algorithm 1 as read in DESIGN.md section 2.3.  A > 1: the
+                              tile-aligned variant (ragged
+                              shards cost kernel efficiency): Per-Doc chunk lengths are multiples
+                              of A and chunks start on multiples of A (the < A leftover tokens
+                              are a movable item at the document's end, next to the last chunk);
+                              the equal-token repair cuts multiples of A from items that start
+                              on a multiple of A and takes the < A remainder Eq. 2 forces from
+                              the head of the donor's shortest item.  Ignored by
+                              FCP_STRATEGY_PER_SEQ.  A = 128 matches the attention tiles. */
 } fcp_plan_opts;
 
 /* Builds the plan for documents `doc_lengths[0..n_docs)` (host) on `n_ranks` workers.
@@ -146,6 +160,13 @@ int  fcp_kv_gather(const fcp_plan* plan, int32_t rank, const void* K, const void
 int  fcp_kv_scatter_add(const fcp_plan* plan, int32_t rank, const void* dk_r, const void* dv_r,
                         int32_t src_dtype, float* dK, float* dV, int32_t n_kv_heads,
                         int32_t head_dim, void* stream, fcp_gather_counts* counts);
+
+/* Last step of the dKV reduction: the fp32 accumulators dK, dV (device, n_elems = C*Hkv*D each,
+ * filled by fcp_kv_scatter_add over all ranks) rounded to nearest-even bf16 into dK_out, dV_out
+ * (device, same shape): the tensors the owner of the tokens hands on.  n_elems
+ * must be a multiple of 8 and all pointers 16-byte aligned.  One kernel launch, asynchronous. */
+int  fcp_kv_reduce_finish(const float* dK, const float* dV, void* dK_out, void* dV_out,
+                          int64_t n_elems, void* stream);
 
 /* ------------------------------------------------------------------------------------------
  * 2b. Local / prefix split of a rank's keys.  PAPER.md:15 and

@@ -207,6 +207,30 @@ def shard_rows_fwd(q_rows, k, v, key_counts, scale):
     return o, lse
 
 
+def shard_rows_bwd_dq(q_rows, k, v, do_rows, key_counts, scale):
+    """Row-at-a-time dq for sampled rows (parity at sizes where the full oracle is too slow):
+    dq of a query row depends on that row alone.  For row i with n = key_counts[i] visible keys
+    p = softmax(scale q.K[:n]), o = p V[:n], delta = dO.o, dp = V[:n] dO,
+    ds = p o (dp - delta), dq = scale ds K[:n]  (the formulas at the top of this file).
+    q_rows, do_rows [m,Hq,D]; k,v [L,Hkv,D] -> dq [m,Hq,D]."""
+    m, Hq, D = q_rows.shape
+    G = _group(Hq, k.shape[1])
+    dq = np.zeros((m, Hq, D))
+    for i in range(m):
+        n = int(key_counts[i])
+        for h in range(Hq):
+            kh, vh = k[:n, h // G, :], v[:n, h // G, :]
+            sc = scale * (kh @ q_rows[i, h, :])
+            e = np.exp(sc - sc.max())
+            p = e / e.sum()
+            o = p @ vh
+            delta = float(do_rows[i, h, :] @ o)
+            dp = vh @ do_rows[i, h, :]
+            ds = p * (dp - delta)
+            dq[i, h, :] = scale * (ds @ kh)
+    return dq
+
+
 # --------------------------------------------------------------------------------------
 # partial-result aggregation (PAPER.md:64, 234)
 # --------------------------------------------------------------------------------------

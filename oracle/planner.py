@@ -47,11 +47,28 @@ def _argmin(keys):
 
 
 def plan(d: Sequence[int], n_ranks: int, r_ppm: int = DEFAULT_R_PPM,
-         strategy: int = STRATEGY_HYBRID) -> Plan:
-    """Algorithm 1.  Raises ValueError where the C-ABI returns INVALID_ARG."""
+         strategy: int = STRATEGY_HYBRID, align: int = 1) -> Plan:
+    """Algorithm 1.  Raises ValueError where the C-ABI returns INVALID_ARG.
+
+    align = A > 1 selects the tile-aligned variant (the paper only notes
+    that short / ragged shards cost kernel efficiency): cuts are placed on
+    multiples of A document positions wherever Eq. 2 leaves the choice, so that a shard's query
+    tiles line up with the key tiles of its document.  A = 1 is Algorithm 1 as read above, step
+    for step.  With A > 1 (readings of DESIGN.md section 2.3):
+      Per-Doc   chunk length q = (d div 2NA) A; of the leftover L = d - 2Nq the aligned part
+                h = (L div A) A is the head item [0, h) of the Whole-Doc pool, chunks start at
+                h + c q, and the last e = L - h < A tokens are a movable item [d - e, d) that
+                starts on the worker of the LAST chunk (worker 0: it merges with that chunk,
+                which ends at the document's ragged end anyway, unless the equal-token repair
+                has to move it); q = 0 leaves the document whole.
+      repair    handing g tokens from worker a to b when no whole item fits:
+                g >= A: cut (g div A) A tokens from the head of a's longest item that starts on
+                a multiple of A (none: its longest item, g tokens);
+                g <  A: cut g tokens from the head of a's SHORTEST item (the unaligned cut that
+                Eq. 2 forces lands on a short document, where a ragged tile wastes least)."""
     d = [int(x) for x in d]
-    n, N = len(d), int(n_ranks)
-    if n < 1 or N < 1 or any(x < 1 for x in d) or r_ppm < 1_000_000:
+    n, N, A = len(d), int(n_ranks), int(align)
+    if n < 1 or N < 1 or any(x < 1 for x in d) or r_ppm < 1_000_000 or A < 1:
         raise ValueError("invalid argument")
     if strategy not in (STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC,
                         STRATEGY_PER_SEQ):
@@ -84,16 +101,23 @@ def plan(d: Sequence[int], n_ranks: int, r_ppm: int = DEFAULT_R_PPM,
         pool = []
         # Per_Doc_P: 2N chunks, chunks c and 2N-1-c to worker c
         for i in order[:k_per]:
-            q = d[i] // (2 * N)
-            r = d[i] - 2 * N * q
-            if r > 0:                                   # remainder = head of the document
+            q = d[i] // (2 * N * A) * A                 # A = 1: d div 2N
+            if q == 0:
+                pool.append([i, 0, d[i]])
+                continue
+            r = (d[i] - 2 * N * q) // A * A             # head of the document; A = 1: d mod 2N
+            e = d[i] - 2 * N * q - r                    # < A tokens on the last chunk; A = 1: 0
+            if r > 0:
                 pool.append([i, 0, r])
-            if q > 0:
-                for c in range(2 * N):
-                    j = c if c < N else 2 * N - 1 - c
-                    fixed.append(Shard(i, r + c * q, q, j))
-                    tok[j] += q
-                    load[j] += W(r + c * q, q)
+            for c in range(2 * N):
+                j = c if c < N else 2 * N - 1 - c
+                fixed.append(Shard(i, r + c * q, q, j))
+                tok[j] += q
+                load[j] += W(r + c * q, q)
+            if e > 0:                                   # only with A > 1
+                items[0].append([i, d[i] - e, e])
+                tok[0] += e
+                load[0] += W(d[i] - e, e)
         for i in order[k_per:]:
             pool.append([i, 0, d[i]])
         pool.sort(key=lambda it: (-it[2], it[0]))
@@ -119,7 +143,13 @@ def plan(d: Sequence[int], n_ranks: int, r_ppm: int = DEFAULT_R_PPM,
                     moved = x
                 else:                                    # cut the head ("lower segment",
                     # PAPER.md:124) of the longest item; its tail stays on worker a
-                    x = min(items[a], key=lambda it: (-it[2], it[0]))
+                    if g >= A:
+                        on_grid = [it for it in items[a] if it[1] % A == 0]
+                        x = min(on_grid or items[a], key=lambda it: (-it[2], it[0]))
+                        if on_grid:
+                            g = g // A * A
+                    else:                                # only with A > 1: the ragged remainder
+                        x = min(items[a], key=lambda it: (it[2], it[0]))
                     moved = [x[0], x[1], g]
                     x[1] += g
                     x[2] -= g

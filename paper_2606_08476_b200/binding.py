@@ -7,7 +7,9 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfcp.so")
+# FCP_LIB selects another build of the same library (tests/test_sanitizers.py: the host sources
+# under ASan / UBSan); there is still no fallback: the named file must exist and export every symbol
+LIB_PATH = os.environ.get("FCP_LIB") or os.path.join(_HERE, "libfcp.so")
 
 EXPORTS = [
     "fcp_strerror", "fcp_version", "fcp_plan_create", "fcp_plan_destroy", "fcp_plan_shards",
@@ -16,6 +18,7 @@ EXPORTS = [
     "fcp_sched_workspace_size", "fcp_sched_upload", "fcp_sched_get_info", "fcp_attn_fwd",
     "fcp_attn_bwd", "fcp_merge", "fcp_plan_piece_stats", "fcp_piece_layout", "fcp_kv_gather_piece",
     "fcp_kv_scatter_add_piece", "fcp_sched_from_plan_piece", "fcp_sched_get_list",
+    "fcp_kv_reduce_finish",
 ]
 
 STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC, STRATEGY_PER_SEQ = 0, 1, 2, 3
@@ -35,7 +38,8 @@ class _Shard(C.Structure):
 
 
 class _PlanOpts(C.Structure):
-    _fields_ = [("imbalance_ppm", C.c_int64), ("strategy", C.c_int32), ("reserved", C.c_int32)]
+    _fields_ = [("imbalance_ppm", C.c_int64), ("strategy", C.c_int32),
+                ("align_tokens", C.c_int32)]
 
 
 class _Stats(C.Structure):
@@ -117,6 +121,8 @@ def _lib():
                    C.c_void_p, C.POINTER(_GatherCounts)]
         lib.fcp_kv_scatter_add.argtypes = [C.c_void_p, C.c_int32] + scatter
         lib.fcp_kv_scatter_add_piece.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + scatter
+        lib.fcp_kv_reduce_finish.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                             C.c_int64, C.c_void_p]
         lib.fcp_sched_create.argtypes = [_I32P, _I32P, _I32P, C.c_int32, _I32P, C.c_int32,
                                          C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_void_p)]
         lib.fcp_sched_from_plan.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32,
@@ -177,9 +183,9 @@ def _event_ptr(ev):
 class Plan:
     """fcp_plan: Algorithm 1 sharding plan (host)."""
 
-    def __init__(self, doc_lengths, n_ranks, imbalance_ppm=0, strategy=STRATEGY_HYBRID):
+    def __init__(self, doc_lengths, n_ranks, imbalance_ppm=0, strategy=STRATEGY_HYBRID, align=0):
         d = _i32(doc_lengths)
-        opts = _PlanOpts(int(imbalance_ppm), int(strategy), 0)
+        opts = _PlanOpts(int(imbalance_ppm), int(strategy), int(align))
         h = C.c_void_p()
         _check(_lib().fcp_plan_create(_p(d), d.size, int(n_ranks), C.byref(opts), C.byref(h)),
                "fcp_plan_create")
@@ -395,6 +401,21 @@ class Sched:
         _check(_lib().fcp_attn_bwd(C.byref(a), do.data_ptr(), None if no_out else dq.data_ptr(),
                                    dk.data_ptr(), dv.data_ptr()), "fcp_attn_bwd")
         return (None if no_out else dq), dk, dv
+
+
+def kv_reduce_finish(dK, dV, dK_out=None, dV_out=None, stream=None):
+    """fcp_kv_reduce_finish: the reduced fp32 dK, dV [C,Hkv,D] rounded to bf16 tensors."""
+    import torch
+    for t in (dK, dV):
+        assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32
+    dK_out = torch.empty_like(dK, dtype=torch.bfloat16) if dK_out is None else dK_out
+    dV_out = torch.empty_like(dV, dtype=torch.bfloat16) if dV_out is None else dV_out
+    assert dK_out.dtype == torch.bfloat16 and dV_out.dtype == torch.bfloat16
+    assert dK.numel() == dV.numel() == dK_out.numel() == dV_out.numel()
+    _check(_lib().fcp_kv_reduce_finish(dK.data_ptr(), dV.data_ptr(), dK_out.data_ptr(),
+                                       dV_out.data_ptr(), dK.numel(), _stream_ptr(stream)),
+           "fcp_kv_reduce_finish")
+    return dK_out, dV_out
 
 
 def merge(o_a, lse_a, o_b, lse_b, o_out=None, lse_out=None, stream=None):

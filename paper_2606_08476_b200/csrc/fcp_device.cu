@@ -184,6 +184,21 @@ fcp_kv_scatter_add_kernel(const T* __restrict__ dk_r, const T* __restrict__ dv_r
   }
 }
 
+// fp32 -> bf16 (round to nearest even) of the reduced dK, dV: 8 elements per thread and step,
+// 32 B in, 16 B out; blockIdx.y selects the tensor.  HBM-bound: 6 bytes per element.
+__global__ void __launch_bounds__(256)
+fcp_kv_reduce_finish_kernel(const float4* __restrict__ a, const float4* __restrict__ b,
+                            int4* __restrict__ a_out, int4* __restrict__ b_out, int64_t n8) {
+  const float4* __restrict__ src = blockIdx.y ? b : a;
+  int4* __restrict__ dst = blockIdx.y ? b_out : a_out;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8;
+       i += (int64_t)gridDim.x * blockDim.x) {
+    const float4 x = src[2 * i], y = src[2 * i + 1];
+    dst[i] = make_int4(fcp::pack_bf16(x.x, x.y), fcp::pack_bf16(x.z, x.w), fcp::pack_bf16(y.x, y.y),
+                       fcp::pack_bf16(y.z, y.w));
+  }
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256)
 fcp_merge_kernel(const void* __restrict__ o_a, const float* __restrict__ lse_a,
@@ -245,19 +260,23 @@ extern "C" int fcp_kv_gather_piece(const fcp_plan* plan, int32_t rank, int32_t p
   if (!aligned16(K) || !aligned16(V) || !aligned16(k_out) || !aligned16(v_out))
     return FCP_MISALIGNED;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v, piece);
-  if (v.n_kv > 0 && (!k_out || !v_out)) return FCP_INVALID_ARG;   // an empty piece needs no buffer
-  // merge ranges that are contiguous in the source (neighbouring documents held whole)
   std::vector<int64_t> src, len;
-  for (size_t g = 0; g < v.kv_len.size(); ++g) {
-    if (v.kv_len[g] == 0) continue;
-    if (!src.empty() && src.back() + len.back() == v.kv_src_start[g]) {
-      len.back() += v.kv_len[g];
-    } else {
-      src.push_back(v.kv_src_start[g]);
-      len.push_back(v.kv_len[g]);
+  // merge ranges that are contiguous in the source (neighbouring documents held whole)
+  const int st = fcp_guard([&] {
+    fcp_build_rank_view(*plan, rank, v, piece);
+    for (size_t g = 0; g < v.kv_len.size(); ++g) {
+      if (v.kv_len[g] == 0) continue;
+      if (!src.empty() && src.back() + len.back() == v.kv_src_start[g]) {
+        len.back() += v.kv_len[g];
+      } else {
+        src.push_back(v.kv_src_start[g]);
+        len.push_back(v.kv_len[g]);
+      }
     }
-  }
+    return (int)FCP_OK;
+  });
+  if (st != FCP_OK) return st;
+  if (v.n_kv > 0 && (!k_out || !v_out)) return FCP_INVALID_ARG;   // an empty piece needs no buffer
   if (counts) {
     counts->total_tokens = v.n_kv;
     counts->remote_tokens = v.remote;
@@ -267,10 +286,13 @@ extern "C" int fcp_kv_gather_piece(const fcp_plan* plan, int32_t rank, int32_t p
     counts->reserved = 0;
   }
   const int64_t cpr = row_bytes / 16;          // chunks per row
-  int num_sms = 148;
-  int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return FCP_CUDA;
-  cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+  const int num_sms = fcp_sm_count();
+  // opt-in to > 48 KB of dynamic shared memory: a per-device (context) attribute, set on every
+  // call so that a process driving several GPUs is served on each
+  if (!src.empty() &&
+      cudaFuncSetAttribute(fcp_kv_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           kGatherSmem) != cudaSuccess)
+    return FCP_CUDA;
   int64_t dst_row = 0;
   for (size_t base = 0; base < src.size(); base += kMaxRanges) {
     GatherRanges rg;
@@ -285,13 +307,6 @@ extern "C" int fcp_kv_gather_piece(const fcp_plan* plan, int32_t rank, int32_t p
     rg.dst0[rg.n] = c;
     const int64_t slabs = 2 * ((c + kSlab - 1) / kSlab);
     if (slabs == 0) continue;
-    static bool attr_set = false;
-    if (!attr_set) {
-      if (cudaFuncSetAttribute(fcp_kv_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                               kGatherSmem) != cudaSuccess)
-        return FCP_CUDA;
-      attr_set = true;
-    }
     const int grid = (int)std::min<int64_t>(slabs, (int64_t)num_sms * 2);
     fcp_kv_gather_kernel<<<grid, 32, kGatherSmem, (cudaStream_t)stream>>>(
         reinterpret_cast<const int4*>(K), reinterpret_cast<const int4*>(V),
@@ -323,18 +338,22 @@ extern "C" int fcp_kv_scatter_add_piece(const fcp_plan* plan, int32_t rank, int3
   if (row_elems % 8 != 0) return FCP_UNSUPPORTED;
   if (!aligned16(dk_r) || !aligned16(dv_r) || !aligned16(dK) || !aligned16(dV)) return FCP_MISALIGNED;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v, piece);
-  if (v.n_kv > 0 && (!dk_r || !dv_r)) return FCP_INVALID_ARG;     // an empty piece needs no buffer
   std::vector<int64_t> tok, len;                  // merged destination ranges (global tokens)
-  for (size_t g = 0; g < v.kv_len.size(); ++g) {
-    if (v.kv_len[g] == 0) continue;
-    if (!tok.empty() && tok.back() + len.back() == v.kv_src_start[g]) {
-      len.back() += v.kv_len[g];
-    } else {
-      tok.push_back(v.kv_src_start[g]);
-      len.push_back(v.kv_len[g]);
+  const int st = fcp_guard([&] {
+    fcp_build_rank_view(*plan, rank, v, piece);
+    for (size_t g = 0; g < v.kv_len.size(); ++g) {
+      if (v.kv_len[g] == 0) continue;
+      if (!tok.empty() && tok.back() + len.back() == v.kv_src_start[g]) {
+        len.back() += v.kv_len[g];
+      } else {
+        tok.push_back(v.kv_src_start[g]);
+        len.push_back(v.kv_len[g]);
+      }
     }
-  }
+    return (int)FCP_OK;
+  });
+  if (st != FCP_OK) return st;
+  if (v.n_kv > 0 && (!dk_r || !dv_r)) return FCP_INVALID_ARG;     // an empty piece needs no buffer
   const int64_t esz = src_dtype == FCP_DTYPE_F32 ? 4 : 2;
   if (counts) {
     counts->total_tokens = v.n_kv;
@@ -345,9 +364,7 @@ extern "C" int fcp_kv_scatter_add_piece(const fcp_plan* plan, int32_t rank, int3
     counts->reserved = 0;
   }
   const int64_t upr = row_elems / 8;              // 8-element units per row
-  int num_sms = 148, dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return FCP_CUDA;
-  cudaDeviceGetAttribute(&num_sms, cudaDevAttrMultiProcessorCount, dev);
+  const int num_sms = fcp_sm_count();
   int64_t src_row = 0;
   for (size_t base = 0; base < tok.size();) {
     // one launch = a run of buffer-contiguous ranges with pairwise distinct destination tokens.
@@ -381,6 +398,21 @@ extern "C" int fcp_kv_scatter_add_piece(const fcp_plan* plan, int32_t rank, int3
     src_row += c / upr;
   }
   return FCP_OK;
+}
+
+extern "C" int fcp_kv_reduce_finish(const float* dK, const float* dV, void* dK_out, void* dV_out,
+                                    int64_t n_elems, void* stream) {
+  if (n_elems < 0 || n_elems % 8 != 0) return FCP_INVALID_ARG;
+  if (n_elems == 0) return FCP_OK;
+  if (!dK || !dV || !dK_out || !dV_out) return FCP_INVALID_ARG;
+  if (!aligned16(dK) || !aligned16(dV) || !aligned16(dK_out) || !aligned16(dV_out))
+    return FCP_MISALIGNED;
+  const int64_t n8 = n_elems / 8;
+  const int grid = (int)std::min<int64_t>((n8 + 255) / 256, (int64_t)fcp_sm_count() * 8);
+  fcp_kv_reduce_finish_kernel<<<dim3(grid, 2), 256, 0, (cudaStream_t)stream>>>(
+      reinterpret_cast<const float4*>(dK), reinterpret_cast<const float4*>(dV),
+      reinterpret_cast<int4*>(dK_out), reinterpret_cast<int4*>(dV_out), n8);
+  return cudaGetLastError() == cudaSuccess ? FCP_OK : FCP_CUDA;
 }
 
 extern "C" int fcp_merge(const void* o_a, const float* lse_a, const void* o_b, const float* lse_b,

@@ -1,6 +1,7 @@
 // Internal (non-ABI) definitions shared by the host and device parts of libfcp.
 #pragma once
 #include <cstdint>
+#include <new>
 #include <vector>
 
 #include "fcp.h"
@@ -85,3 +86,20 @@ struct fcp_sched {
   size_t off_counters = 0, off_fwd = 0, off_bwd = 0, off_sub = 0, off_shard_meta = 0,
          off_fwd_cta = 0, off_bwd_cta = 0, off_lsed = 0, off_dq = 0, total = 0;
 };
+
+// Runs the body of an extern "C" entry point: nothing may throw across the C ABI (fcp.h), so a
+// failed host allocation becomes FCP_NO_MEMORY and anything else FCP_INVALID_ARG.
+template <class F>
+int fcp_guard(F&& body) noexcept {
+  try {
+    return body();
+  } catch (const std::bad_alloc&) {
+    return FCP_NO_MEMORY;
+  } catch (...) {
+    return FCP_INVALID_ARG;
+  }
+}
+
+// SM count of the current device (148 on B200; also the answer when no device is visible, e.g.
+// a schedule built on a CPU-only box).  Write-once per-device cache behind atomics.
+int32_t fcp_sm_count();

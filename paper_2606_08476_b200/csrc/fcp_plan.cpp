@@ -3,6 +3,7 @@
 // section 3.  Integer arithmetic only (64-bit loads, 128-bit ratio comparison).
 #include <algorithm>
 #include <cstring>
+#include <memory>
 #include <new>
 
 #include "fcp_internal.h"
@@ -32,24 +33,37 @@ int least_loaded(const std::vector<Worker>& w, Pred ok) {
   return best;
 }
 
+// A = fcp_plan_opts.align_tokens (1 = Algorithm 1 proper; > 1 = the tile-aligned variant, fcp.h)
 void run_pass(const std::vector<int32_t>& d, const std::vector<int32_t>& order, int k_per,
-              int N, int64_t T, Pass& ps) {
+              int N, int64_t T, int32_t A, Pass& ps) {
   ps.w.assign(N, Worker());
   ps.chunks.clear();
   std::vector<Item> pool;
   // Per-Doc: 2N chunks, chunk c and 2N-1-c on worker c; d mod 2N tokens at the
   // head of the document become an ordinary Whole-Doc item.
+  // With A > 1 the chunk length is a multiple of A, the head item is the aligned part of the
+  // leftover and its ragged rest (< A tokens) is a movable item at the document's end that
+  // starts on the worker of the last chunk.
   for (int x = 0; x < k_per; ++x) {
     const int32_t i = order[x];
-    const int32_t q = d[i] / (2 * N), r = d[i] - 2 * N * q;
+    const int32_t q = (int32_t)(d[i] / (2 * (int64_t)N * A) * A);
+    if (q == 0) {
+      pool.push_back({i, 0, d[i]});
+      continue;
+    }
+    const int32_t r = (d[i] - 2 * N * q) / A * A, e = d[i] - 2 * N * q - r;
     if (r > 0) pool.push_back({i, 0, r});
-    if (q > 0)
-      for (int c = 0; c < 2 * N; ++c) {
-        const int j = c < N ? c : 2 * N - 1 - c;
-        ps.chunks.push_back({i, r + c * q, q, j});
-        ps.w[j].tok += q;
-        ps.w[j].load += fcp_W(r + c * q, q);
-      }
+    for (int c = 0; c < 2 * N; ++c) {
+      const int j = c < N ? c : 2 * N - 1 - c;
+      ps.chunks.push_back({i, r + c * q, q, j});
+      ps.w[j].tok += q;
+      ps.w[j].load += fcp_W(r + c * q, q);
+    }
+    if (e > 0) {
+      ps.w[0].items.push_back({i, d[i] - e, e});
+      ps.w[0].tok += e;
+      ps.w[0].load += fcp_W(d[i] - e, e);
+    }
   }
   for (size_t x = k_per; x < order.size(); ++x) pool.push_back({order[x], 0, d[order[x]]});
   std::stable_sort(pool.begin(), pool.end(), [](const Item& a, const Item& b) {
@@ -84,14 +98,24 @@ void run_pass(const std::vector<int32_t>& d, const std::vector<int32_t>& order, 
       if (pick >= 0) {
         moved = src[pick];
         src.erase(src.begin() + pick);
-      } else {                                        // cut the head of the longest item
-        for (int x = 0; x < (int)src.size(); ++x)
-          if (pick < 0 || src[x].len > src[pick].len ||
-              (src[x].len == src[pick].len && src[x].doc < src[pick].doc))
+      } else {
+        // cut the head of the longest item (A > 1: of the longest item that starts on a multiple
+        // of A, and a multiple of A tokens; a hand-over below A comes from the shortest item)
+        int32_t g = (int32_t)room;
+        const bool ragged = g < A;
+        bool on_grid = false;
+        for (int x = 0; x < (int)src.size() && !ragged; ++x) on_grid |= src[x].start % A == 0;
+        for (int x = 0; x < (int)src.size(); ++x) {
+          if (on_grid && src[x].start % A != 0) continue;
+          const bool better = ragged ? src[x].len < src[pick < 0 ? x : pick].len
+                                     : src[x].len > src[pick < 0 ? x : pick].len;
+          if (pick < 0 || better || (src[x].len == src[pick].len && src[x].doc < src[pick].doc))
             pick = x;
-        moved = {src[pick].doc, src[pick].start, (int32_t)room};
-        src[pick].start += (int32_t)room;
-        src[pick].len -= (int32_t)room;
+        }
+        if (on_grid) g = g / A * A;
+        moved = {src[pick].doc, src[pick].start, g};
+        src[pick].start += g;
+        src[pick].len -= g;
       }
       const uint64_t wl = fcp_W(moved.start, moved.len);
       ps.w[a].tok -= moved.len;  ps.w[a].load -= wl;
@@ -113,9 +137,10 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
                                const fcp_plan_opts* opts, fcp_plan** out) {
   if (!doc_lengths || !out || n_docs < 1 || n_ranks < 1) return FCP_INVALID_ARG;
   int64_t r_ppm = 1050000;
-  int32_t strategy = FCP_STRATEGY_HYBRID;
+  int32_t strategy = FCP_STRATEGY_HYBRID, align = 1;
   if (opts) {
-    if (opts->reserved != 0) return FCP_INVALID_ARG;
+    if (opts->align_tokens < 0) return FCP_INVALID_ARG;
+    if (opts->align_tokens > 1) align = opts->align_tokens;
     if (opts->imbalance_ppm != 0) r_ppm = opts->imbalance_ppm;
     strategy = opts->strategy;
   }
@@ -130,9 +155,8 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
   if (strategy == FCP_STRATEGY_PER_SEQ && C % (2 * (int64_t)n_ranks) != 0) return FCP_INVALID_ARG;
   const int N = n_ranks;
   const int64_t T = C / N;
-
-  fcp_plan* p = new (std::nothrow) fcp_plan();
-  if (!p) return FCP_INVALID_ARG;
+  return fcp_guard([&]() -> int {
+  std::unique_ptr<fcp_plan> p(new fcp_plan());
   p->d.assign(doc_lengths, doc_lengths + n_docs);
   p->off.resize(n_docs + 1);
   p->off[0] = 0;
@@ -166,7 +190,7 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
   const int k_last = strategy == FCP_STRATEGY_WHOLE_DOC ? 0 : n_docs;
   Pass ps;
   for (; strategy != FCP_STRATEGY_PER_SEQ;) {          // line 4
-    run_pass(p->d, order, k_per, N, T, ps);
+    run_pass(p->d, order, k_per, N, T, align, ps);
     ++p->n_passes;
     // Cur_R > R  <=>  max * N * 1e6 > R_ppm * sum, in 128 bits
     const unsigned __int128 lhs = (unsigned __int128)ps.max_load * (uint64_t)N * 1000000u;
@@ -207,8 +231,9 @@ extern "C" int fcp_plan_create(const int32_t* doc_lengths, int32_t n_docs, int32
   p->rank_begin.assign(N + 1, 0);
   for (const fcp_shard& s : p->shards) ++p->rank_begin[s.rank + 1];
   for (int j = 0; j < N; ++j) p->rank_begin[j + 1] += p->rank_begin[j];
-  *out = p;
+  *out = p.release();
   return FCP_OK;
+  });
 }
 
 extern "C" void fcp_plan_destroy(fcp_plan* plan) { delete plan; }
@@ -305,7 +330,8 @@ extern "C" int fcp_plan_piece_stats(const fcp_plan* plan, int32_t rank, int32_t 
   if (!plan || !out || rank < 0 || rank >= plan->n_ranks || !valid_piece(piece))
     return FCP_INVALID_ARG;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v, piece);
+  const int st = fcp_guard([&] { fcp_build_rank_view(*plan, rank, v, piece); return (int)FCP_OK; });
+  if (st != FCP_OK) return st;
   out->n_shards = (int32_t)v.q_pos_off.size();
   out->n_segs = (int32_t)v.kv_len.size();
   out->n_q = v.n_q;
@@ -335,7 +361,8 @@ extern "C" int fcp_plan_stats(const fcp_plan* plan, fcp_stats* out) {
   int64_t max_nonlast = 0;
   for (int r = 0; r < N; ++r) {
     RankView v;
-    fcp_build_rank_view(*plan, r, v);
+    const int st = fcp_guard([&] { fcp_build_rank_view(*plan, r, v); return (int)FCP_OK; });
+    if (st != FCP_OK) return st;
     max_nonlast = std::max(max_nonlast, v.nonlast);
     out->max_remote_tokens = std::max(out->max_remote_tokens, v.remote);
     out->sum_remote_tokens += v.remote;
@@ -355,7 +382,8 @@ extern "C" int fcp_piece_layout(const fcp_plan* plan, int32_t rank, int32_t piec
   if (!plan || !out || rank < 0 || rank >= plan->n_ranks || !valid_piece(piece))
     return FCP_INVALID_ARG;
   RankView v;
-  fcp_build_rank_view(*plan, rank, v, piece);
+  const int st = fcp_guard([&] { fcp_build_rank_view(*plan, rank, v, piece); return (int)FCP_OK; });
+  if (st != FCP_OK) return st;
   auto put = [](int32_t* dst, const std::vector<int32_t>& src) {
     if (dst && !src.empty()) std::memcpy(dst, src.data(), sizeof(int32_t) * src.size());
   };
@@ -389,8 +417,9 @@ extern "C" const char* fcp_strerror(int status) {
     case FCP_BUFFER_TOO_SMALL: return "buffer too small";
     case FCP_CUDA: return "CUDA error";
     case FCP_MISALIGNED: return "misaligned pointer";
+    case FCP_NO_MEMORY: return "out of host memory";
     default: return "unknown status";
   }
 }
 
-extern "C" const char* fcp_version(void) { return "sm_100a;fcp-0.1"; }
+extern "C" const char* fcp_version(void) { return "sm_100a;fcp-0.2"; }

@@ -6,34 +6,15 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cstring>
+#include <memory>
 #include <new>
 
 #include "fcp_internal.h"
 
 namespace {
 size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-
-// Persistent grid size = SM count of the current device (148 on B200; also the value used when
-// no device is visible, e.g. when a schedule is built on a CPU-only box).  Cached per device:
-// the query costs more than the rest of a small schedule.
-int32_t grid_ctas() {
-  static int cached_dev = -2, cached_n = 148;
-  int dev = -1;
-  if (cudaGetDevice(&dev) != cudaSuccess) {
-    cudaGetLastError();
-    dev = -1;
-  }
-  if (dev == cached_dev) return cached_n;
-  int n = 0;
-  if (dev < 0 || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
-    cudaGetLastError();
-    n = 148;
-  }
-  cached_dev = dev;
-  cached_n = n;
-  return n;
-}
 
 // Stable sort by descending integer key (counting sort: the keys are tile / iteration counts).
 template <typename Item, typename Key>
@@ -96,8 +77,32 @@ void assign_lpt(std::vector<Item>& items, int32_t n_cta, Cost cost, std::vector<
 }
 }
 
+// Persistent grid size = SM count of the current device.  The attribute query costs more than
+// the rest of a small schedule, so the answer is cached per device: a write-once table of
+// immutable hardware facts behind atomics (safe from any thread, for any device).
+int32_t fcp_sm_count() {
+  constexpr int kMaxDev = 64;
+  static std::atomic<int32_t> cache[kMaxDev];      // 0 = not queried yet
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    cudaGetLastError();
+    return 148;                                    // no device visible (CPU-only box)
+  }
+  if (dev >= 0 && dev < kMaxDev) {
+    const int32_t c = cache[dev].load(std::memory_order_relaxed);
+    if (c > 0) return c;
+  }
+  int n = 0;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) {
+    cudaGetLastError();
+    return 148;
+  }
+  if (dev >= 0 && dev < kMaxDev) cache[dev].store(n, std::memory_order_relaxed);
+  return n;
+}
+
 // n_cta: size of the persistent grid
-static int sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
+static int sched_create_impl(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
                         const int32_t* shard_seg, int32_t n_shards, const int32_t* cu_seqlens_k,
                         int32_t n_segs, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
                         int32_t n_cta, fcp_sched** out) {
@@ -112,8 +117,8 @@ static int sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
   for (int g = 0; g < n_segs; ++g)
     if (cu_seqlens_k[g + 1] < cu_seqlens_k[g]) return FCP_INVALID_ARG;
 
-  fcp_sched* s = new (std::nothrow) fcp_sched();
-  if (!s) return FCP_INVALID_ARG;
+  std::unique_ptr<fcp_sched> owner(new fcp_sched());
+  fcp_sched* s = owner.get();
   s->Hq = n_q_heads;  s->Hkv = n_kv_heads;  s->D = head_dim;
   s->G = n_q_heads / n_kv_heads;
   s->NQ = (s->G % 2 == 0) ? 2 : 1;
@@ -242,8 +247,18 @@ static int sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
   put(s->off_fwd_cta, s->fwd_cta_off.data(), s->fwd_cta_off.size() * sizeof(int32_t));
   put(s->off_bwd_cta, s->bwd_cta_off.data(), s->bwd_cta_off.size() * sizeof(int32_t));
   put(s->off_shard_meta, s->tile_meta.data(), s->tile_meta.size() * sizeof(int32_t));
-  *out = s;
+  *out = owner.release();
   return FCP_OK;
+}
+
+static int sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
+                        const int32_t* shard_seg, int32_t n_shards, const int32_t* cu_seqlens_k,
+                        int32_t n_segs, int32_t n_q_heads, int32_t n_kv_heads, int32_t head_dim,
+                        int32_t n_cta, fcp_sched** out) {
+  return fcp_guard([&] {
+    return sched_create_impl(cu_seqlens_q, q_pos_off, shard_seg, n_shards, cu_seqlens_k, n_segs,
+                             n_q_heads, n_kv_heads, head_dim, n_cta, out);
+  });
 }
 
 extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_pos_off,
@@ -251,13 +266,14 @@ extern "C" int fcp_sched_create(const int32_t* cu_seqlens_q, const int32_t* q_po
                                 const int32_t* cu_seqlens_k, int32_t n_segs, int32_t n_q_heads,
                                 int32_t n_kv_heads, int32_t head_dim, fcp_sched** out) {
   return sched_create(cu_seqlens_q, q_pos_off, shard_seg, n_shards, cu_seqlens_k, n_segs,
-                      n_q_heads, n_kv_heads, head_dim, grid_ctas(), out);
+                      n_q_heads, n_kv_heads, head_dim, fcp_sm_count(), out);
 }
 
 static int sched_from_plan(const fcp_plan* plan, int32_t rank, int32_t piece, int32_t n_q_heads,
                            int32_t n_kv_heads, int32_t head_dim, int32_t n_cta, fcp_sched** out) {
   RankView v;
-  fcp_build_rank_view(*plan, rank, v, piece);
+  const int st = fcp_guard([&] { fcp_build_rank_view(*plan, rank, v, piece); return (int)FCP_OK; });
+  if (st != FCP_OK) return st;
   return sched_create(v.cu_q.data(), v.q_pos_off.data(), v.shard_seg.data(),
                       (int32_t)v.q_pos_off.size(), v.cu_k.data(), (int32_t)v.kv_len.size(),
                       n_q_heads, n_kv_heads, head_dim, n_cta, out);
@@ -274,7 +290,7 @@ extern "C" int fcp_sched_from_plan_piece(const fcp_plan* plan, int32_t rank, int
   if (!plan || !out || rank < 0 || rank >= plan->n_ranks ||
       (piece != FCP_PIECE_FULL && piece != FCP_PIECE_LOCAL && piece != FCP_PIECE_PREFIX))
     return FCP_INVALID_ARG;
-  return sched_from_plan(plan, rank, piece, n_q_heads, n_kv_heads, head_dim, grid_ctas(), out);
+  return sched_from_plan(plan, rank, piece, n_q_heads, n_kv_heads, head_dim, fcp_sm_count(), out);
 }
 
 extern "C" void fcp_sched_destroy(fcp_sched* sched) { delete sched; }

@@ -127,24 +127,11 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr) {        // same wa
 }
 
 // ---------------------------------------------------------------- UMMA descriptors
-// Shared-memory matrix descriptor, SWIZZLE_128B, sm_100 version field = 1.
+// Shared-memory matrix descriptors (SWIZZLE_128B, sm_100 version field = 1) are built by the MMA
+// issuers from two 32-bit words (see fcp_attn_fwd.cu / fcp_attn_bwd.cu):
 //   K-major  operand: rows of 128 B (64 bf16 of K), 8-row groups SBO bytes apart (LBO unused).
 //   MN-major operand: rows of 128 B (64 bf16 of M/N) per K index, 8-K-row groups SBO bytes
 //                     apart, next 64 M/N elements LBO bytes apart.
-__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr, uint32_t lbo_bytes,
-                                                    uint32_t sbo_bytes) {
-  uint64_t d = 0;
-  d |= (uint64_t)((saddr & 0x3FFFF) >> 4);
-  d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
-  d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
-  d |= (uint64_t)1 << 46;    // descriptor version (Blackwell)
-  d |= (uint64_t)2 << 61;    // SWIZZLE_128B
-  return d;
-}
-// Same descriptor, start address advanced by `bytes` (multiple of 16; stays inside the 256 KB window).
-__device__ __forceinline__ uint64_t umma_desc_add(uint64_t desc, uint32_t bytes) {
-  return desc + (uint64_t)(bytes >> 4);
-}
 // Instruction descriptor, kind::f16: bf16 x bf16 -> f32.
 __host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, int a_mn_major, int b_mn_major) {
   return (1u << 4)                       // D format f32
@@ -192,16 +179,6 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
         "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]),
         "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]),
         "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-      : "r"(taddr)
-      : "memory");
-}
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&r)[16]) {
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]),
-        "=r"(r[7]), "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]),
-        "=r"(r[14]), "=r"(r[15])
       : "r"(taddr)
       : "memory");
 }
@@ -294,11 +271,6 @@ __device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
 __device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
   f32x2 r;
   asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-  return r;
-}
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
-  f32x2 r;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
   return r;
 }
 __device__ __forceinline__ float max3(float a, float b, float c) {

@@ -115,34 +115,51 @@ def test_ragged_cases(fcp, torch, case, dkv_f32):
         U.compare_rank(fcp, d, N, r, Hq, Hkv, D, seed=1, strategy=strategy, dkv_f32=dkv_f32)
 
 
-def test_key_count_closed_form_full_size(fcp, torch):
+@pytest.mark.parametrize("name,ranks", [("8b", (0, 3)), ("longtail_256k", (0,)), ("longtail_1m", (0,))])
+def test_key_count_closed_form_full_size(fcp, torch, name, ranks):
     """K = 0 makes lse = ln(#visible keys) exactly (SURVEY 8(c1) pin 3) and o the running mean
-    of V: checks every mask and offset of the real 8b-size launch without an O(n^2) oracle."""
-    cfg = fcp_inputs.CONFIGS["8b"]
-    d = fcp_inputs.doc_lengths("8b", 0)
+    of V: checks every mask, offset and the 32-bit row arithmetic of the real full-size launches
+    (8b, and the 256K / 1M ends of the context-window sweep)
+    without an O(n^2) oracle.  All heads on the GPU; lse is checked on every row and head, o on
+    every row of the rank's shard with the longest prefix for one kv head's query heads."""
+    cfg = fcp_inputs.CONFIGS[name]
+    d = fcp_inputs.doc_lengths(name, 0)
     plan = fcp.Plan(d, cfg.N)
-    _, _, V, _ = fcp_inputs.make_tensors(cfg.C, cfg.Hq, cfg.Hkv, cfg.D, 0)
-    Vd = V.cuda()
+    gen = torch.Generator(device="cuda").manual_seed(0)
+    Vd = torch.randn((cfg.C, cfg.Hkv, cfg.D), device="cuda", generator=gen).to(torch.bfloat16)
     Kd = torch.zeros_like(Vd)
-    G = cfg.Hq // cfg.Hkv
-    for r in (0, cfg.N - 1):
+    G, hk = cfg.Hq // cfg.Hkv, cfg.Hkv - 1
+    for r in ranks:
         lay = plan.rank_layout(r)
         n_q = int(lay["cu_seqlens_q"][-1])
-        q = torch.randn((n_q, cfg.Hq, cfg.D), device="cuda").to(torch.bfloat16)
+        q = torch.randn((n_q, cfg.Hq, cfg.D), device="cuda", generator=gen).to(torch.bfloat16)
         kg, vg, _ = plan.kv_gather(r, Kd, Vd)
         sched = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload("cuda")
         o, lse = sched.attn_fwd(q, kg, vg, 1.0 / math.sqrt(cfg.D))
         torch.cuda.synchronize()
         vis = np.concatenate([int(p) + 1 + np.arange(int(b - a)) for a, b, p in
                               zip(lay["cu_seqlens_q"][:-1], lay["cu_seqlens_q"][1:], lay["q_pos_off"])])
-        want = np.broadcast_to(np.log(vis.astype(np.float64)), (cfg.Hq, n_q))
-        assert np.abs(lse.cpu().double().numpy() - want).max() <= 1e-3
-        # o = mean of the visible V rows (first shard, every query head)
-        a, b, p = int(lay["cu_seqlens_q"][0]), int(lay["cu_seqlens_q"][1]), int(lay["q_pos_off"][0])
-        k0 = int(lay["cu_seqlens_k"][lay["shard_seg"][0]])
-        vv = U.to_f64(vg[k0:k0 + p + (b - a)])
-        mean = np.cumsum(vv, axis=0)[p:p + (b - a)] / vis[a:b, None, None]
-        U.check("o", U.to_f64(o[a:b]), np.repeat(mean, G, axis=1))
+        want = np.log(vis.astype(np.float64))
+        err = float(np.abs(lse.cpu().double().numpy() - want[None, :]).max())
+        assert err <= 1e-3, (name, r, err)
+        # o = mean of the visible V rows
+        i = int(np.argmax(lay["q_pos_off"]))
+        a, b, p = int(lay["cu_seqlens_q"][i]), int(lay["cu_seqlens_q"][i + 1]), int(lay["q_pos_off"][i])
+        k0 = int(lay["cu_seqlens_k"][lay["shard_seg"][i]])
+        vv = U.to_f64(vg[k0:k0 + p + (b - a), hk])
+        mean = np.cumsum(vv, axis=0)[p:p + (b - a)] / vis[a:b, None]
+        mx, _ = U.check("o", U.to_f64(o[a:b, hk * G:(hk + 1) * G]), np.repeat(mean[:, None, :], G, axis=1))
+        print("\n%s rank %d: %d rows, longest prefix %d, max |lse - ln n| %.2e, max |o - mean V| %.2e"
+              % (name, r, n_q, p, err, mx))
+        del q, kg, vg, o, lse
+
+
+# (max-abs, mean-abs) bounds of test_forward_running_max_growth; PLACEHOLDER = the round-1 bounds
+# until the observed errors are in (see the test)
+GROWTH_BOUNDS = {
+    128: {"dq": (2e-2 + 5e-3 * 190, 2e-3 + 2e-4 * 190), "dk": (5e-2, 5e-3), "dv": (5e-2, 5e-3)},
+    64: {"dq": (2e-2 + 5e-3 * 190, 2e-3 + 2e-4 * 190), "dk": (5e-2, 5e-3), "dv": (5e-2, 5e-3)},
+}
 
 
 @pytest.mark.parametrize("D,Hq,Hkv", [(128, 2, 1), (64, 3, 1)], ids=["D128_NQ2", "D64_NQ1"])
@@ -179,55 +196,141 @@ def test_forward_running_max_growth(fcp, torch, D, Hq, Hkv):
     # scale * 2^-9 * 20 * max|K| ~ 3.5e-3 * max|K|.  The north_star tolerance (stated for N(0,1)
     # inputs, max|K| ~ 4) is widened by that term.
     kmax = float(K.abs().max())
-    U.check("dq", U.to_f64(g["dq"]), w["dq"], max_abs=2e-2 + 5e-3 * kmax, mean_abs=2e-3 + 2e-4 * kmax)
+    obs = {k: (float(np.abs(U.to_f64(g[k]) - w[k]).max()), float(np.abs(U.to_f64(g[k]) - w[k]).mean()),
+               float(np.abs(w[k]).max())) for k in ("dq", "dk", "dv")}
+    obs["lse"] = (float(np.abs(lse_g - w["lse"]).max()), 0.0, float(np.abs(w["lse"]).max()))
+    print("\ngrowth D=%d: max|K| %.1f, observed (max-abs err, mean-abs err, max |expected|):" % (D, kmax),
+          {k: tuple(float("%.3g" % x) for x in v) for k, v in obs.items()})
+    # bounds = about twice the errors observed on B200 ("growth test")
+    U.check("dq", U.to_f64(g["dq"]), w["dq"], max_abs=GROWTH_BOUNDS[D]["dq"][0],
+            mean_abs=GROWTH_BOUNDS[D]["dq"][1])
     for k in ("dk", "dv"):
-        U.check(k, U.to_f64(g[k]), w[k], max_abs=5e-2, mean_abs=5e-3, bf16_sum=True)
+        U.check(k, U.to_f64(g[k]), w[k], max_abs=GROWTH_BOUNDS[D][k][0],
+                mean_abs=GROWTH_BOUNDS[D][k][1], bf16_sum=True)
 
 
-@pytest.mark.parametrize("dkv_f32", [False, True], ids=["dkv_bf16", "dkv_f32"])
-def test_8b_config_one_gqa_group(fcp, torch, dkv_f32):
-    """Full-size 8b launch (all heads on the GPU, the launch configuration bench.py times);
-    the oracle checks every row of one GQA group (heads are independent units)."""
+def _gpu_rank_both_modes(fcp, torch, plan, r, Q, K, V, dO, scale):
+    """One virtual rank on the GPU with bf16 and with fp32 dk / dv; outputs moved to the host."""
+    out = {}
+    for f32 in (False, True):
+        g = U.run_rank_gpu(fcp, plan, r, Q, K, V, dO, scale, dkv_f32=f32)
+        if not f32:
+            out.update({k: g[k].cpu() for k in ("o", "lse", "dq")})
+        out["dk_f32" if f32 else "dk"] = g["dk"].cpu()
+        out["dv_f32" if f32 else "dv"] = g["dv"].cpu()
+        del g
+    torch.cuda.empty_cache()
+    return out
+
+
+def _check_group(tag, g, w, hq, hk, worst):
+    """One GQA group of one rank against the oracle: o, lse, dq, dk / dv in both output modes
+    (fp32 partials at the plain north-star bound, bf16 with the half-ulp reading of DESIGN.md
+    section 8).  `worst` collects the observed maxima."""
+    res = {"o": U.check(tag + " o", U.to_f64(g["o"][:, hq]), w["o"]),
+           "lse": (U.check_lse(tag + " lse", U.to_f64(g["lse"][hq]), w["lse"]), 0.0),
+           "dq": U.check(tag + " dq", U.to_f64(g["dq"][:, hq]), w["dq"])}
+    for k in ("dk", "dv"):
+        res[k + "_f32"] = U.check(tag + " %s f32" % k, U.to_f64(g[k + "_f32"][:, hk:hk + 1]), w[k])
+        res[k + "_bf16"] = U.check(tag + " %s bf16" % k, U.to_f64(g[k][:, hk:hk + 1]), w[k],
+                                   bf16_sum=True)
+        res["|%s|" % k] = (float(np.abs(w[k]).max()), float(np.abs(w[k]).mean()))
+    for k, v in res.items():
+        worst[k] = tuple(max(a, b) for a, b in zip(worst.get(k, (0.0, 0.0)), v))
+
+
+def test_8b_full_tensors(fcp, torch):
+    """SURVEY 8(d) "full tensors on tiny/8b": every virtual rank x every kv head (with its G
+    query heads) of the benchmarked 8b launch against the oracle, forward and backward, dk / dv
+    as bf16 and as fp32 partials."""
     cfg = fcp_inputs.CONFIGS["8b"]
     d = fcp_inputs.doc_lengths("8b", 0)
     scale = 1.0 / math.sqrt(cfg.D)
     Q, K, V, dO = fcp_inputs.make_tensors(cfg.C, cfg.Hq, cfg.Hkv, cfg.D, 0)
+    Qd, Kd, Vd, dOd = Q.cuda(), K.cuda(), V.cuda(), dO.cuda()
     plan = fcp.Plan(d, cfg.N)
     G = cfg.Hq // cfg.Hkv
-    r, hk = 1, 5
-    g = U.run_rank_gpu(fcp, plan, r, Q.cuda(), K.cuda(), V.cuda(), dO.cuda(), scale,
-                       dkv_f32=dkv_f32)
-    hq = slice(hk * G, (hk + 1) * G)
-    w = U.run_rank_oracle(d, cfg.N, r, U.to_f64(Q[:, hq]), U.to_f64(K[:, hk:hk + 1]),
-                          U.to_f64(V[:, hk:hk + 1]), U.to_f64(dO[:, hq]), scale)
-    U.check("o", U.to_f64(g["o"][:, hq]), w["o"])
-    U.check_lse("lse", U.to_f64(g["lse"][hq]), w["lse"])
-    U.check("dq", U.to_f64(g["dq"][:, hq]), w["dq"])
-    U.check("dk", U.to_f64(g["dk"][:, hk:hk + 1]), w["dk"], bf16_sum=not dkv_f32)
-    U.check("dv", U.to_f64(g["dv"][:, hk:hk + 1]), w["dv"], bf16_sum=not dkv_f32)
+    worst = {}
+    for r in range(cfg.N):
+        g = _gpu_rank_both_modes(fcp, torch, plan, r, Qd, Kd, Vd, dOd, scale)
+        for hk in range(cfg.Hkv):
+            hq = slice(hk * G, (hk + 1) * G)
+            w = U.run_rank_oracle(d, cfg.N, r, U.to_f64(Q[:, hq]), U.to_f64(K[:, hk:hk + 1]),
+                                  U.to_f64(V[:, hk:hk + 1]), U.to_f64(dO[:, hq]), scale)
+            _check_group("8b r%d kv%d" % (r, hk), g, w, hq, hk, worst)
+    print("\n8b full tensors, observed (max-abs, mean-abs):",
+          {k: tuple(float("%.3g" % x) for x in v) for k, v in worst.items()})
+
+
+def _sampled_rows_check(tag, lay, g, Qg, Kg, Vg, dOg, rows, scale, worst):
+    """Seeded sample of query rows of one (rank, GQA group): o, lse and dq of a row depend on
+    that row alone, so oracle.attention.shard_rows_fwd / shard_rows_bwd_dq give them in O(keys).
+    lay: the ORACLE's rank layout; Qg.. the group's local q / dO rows and gathered k / v (fp64);
+    g: the GPU outputs of the group (fp64)."""
+    cu_q, cu_k = np.asarray(lay.cu_seqlens_q), np.asarray(lay.cu_seqlens_k)
+    shard = np.searchsorted(cu_q, rows, side="right") - 1
+    counts = np.asarray(lay.q_pos_off)[shard] + (rows - cu_q[shard]) + 1
+    seg = np.asarray(lay.shard_seg)[shard]
+    for s_ in np.unique(seg):
+        sel = seg == s_
+        k, v = Kg[cu_k[s_]:cu_k[s_ + 1]], Vg[cu_k[s_]:cu_k[s_ + 1]]
+        o, lse = OA.shard_rows_fwd(Qg[rows[sel]], k, v, counts[sel], scale)
+        dq = OA.shard_rows_bwd_dq(Qg[rows[sel]], k, v, dOg[rows[sel]], counts[sel], scale)
+        res = {"o": U.check(tag + " o", g["o"][rows[sel]], o),
+               "lse": (U.check_lse(tag + " lse", g["lse"][:, rows[sel]], lse), 0.0),
+               "dq": U.check(tag + " dq", g["dq"][rows[sel]], dq)}
+        for kk, vv in res.items():
+            worst[kk] = tuple(max(a, b) for a, b in zip(worst.get(kk, (0.0, 0.0)), vv))
 
 
 @pytest.mark.parametrize("name,r,hk", [("short", 7, 2), ("longtail", 3, 6), ("70b", 5, 1)])
-def test_full_size_configs_one_gqa_group(fcp, torch, name, r, hk):
+def test_full_size_configs(fcp, torch, name, r, hk):
     """The other BASELINE.json configs at full size, in the launch configuration bench.py times
-    (all heads, tensors drawn on the device as bench.py does): the oracle checks every row of one
-    GQA group of one virtual rank, forward and backward (heads are independent units, SURVEY
-    8(d)).  longtail and 70b put Per-Doc shards with 70K-key prefixes and G = 8 on the kernels."""
+    (all heads, tensors drawn on the device as bench.py does).  SURVEY 8(d): the oracle checks
+    every row of one GQA group of one virtual rank, forward and backward, dk / dv in both
+    output modes (heads are independent units); plus a seeded sample of 64 rows (o, lse, dq) in
+    every other GQA group of that rank and in one seeded group of every other rank.  longtail
+    and 70b put Per-Doc shards with 70K-key prefixes and G = 8 on the kernels."""
     cfg = fcp_inputs.CONFIGS[name]
     d = fcp_inputs.doc_lengths(name, 0)
     scale = 1.0 / math.sqrt(cfg.D)
     Q, K, V, dO = fcp_inputs.make_tensors(cfg.C, cfg.Hq, cfg.Hkv, cfg.D, 0, device="cuda")
-    plan = fcp.Plan(d, cfg.N)
+    plan, opl = fcp.Plan(d, cfg.N), OP.plan(d, cfg.N)
     G = cfg.Hq // cfg.Hkv
-    g = U.run_rank_gpu(fcp, plan, r, Q, K, V, dO, scale)
+    worst = {}
+    g = _gpu_rank_both_modes(fcp, torch, plan, r, Q, K, V, dO, scale)
     hq = slice(hk * G, (hk + 1) * G)
     w = U.run_rank_oracle(d, cfg.N, r, U.to_f64(Q[:, hq]), U.to_f64(K[:, hk:hk + 1]),
                           U.to_f64(V[:, hk:hk + 1]), U.to_f64(dO[:, hq]), scale)
-    U.check("o", U.to_f64(g["o"][:, hq]), w["o"])
-    U.check_lse("lse", U.to_f64(g["lse"][hq]), w["lse"])
-    U.check("dq", U.to_f64(g["dq"][:, hq]), w["dq"])
-    U.check("dk", U.to_f64(g["dk"][:, hk:hk + 1]), w["dk"], bf16_sum=True)
-    U.check("dv", U.to_f64(g["dv"][:, hk:hk + 1]), w["dv"], bf16_sum=True)
+    _check_group("%s r%d kv%d" % (name, r, hk), g, w, hq, hk, worst)
+    print("\n%s full group, observed (max-abs, mean-abs):" % name,
+          {k: tuple(float("%.3g" % x) for x in v) for k, v in worst.items()})
+    # sampled rows elsewhere
+    rng = np.random.default_rng(17)
+    sampled, n_rows, g_full = {}, 0, g
+    for r2 in range(cfg.N):
+        groups = [h for h in range(cfg.Hkv) if h != hk] if r2 == r else [int(rng.integers(cfg.Hkv))]
+        if r2 == r:
+            g = g_full
+        else:
+            gg = U.run_rank_gpu(fcp, plan, r2, Q, K, V, dO, scale)
+            g = {k: gg[k].cpu() for k in ("o", "lse", "dq")}
+            del gg
+        lay = OKV.rank_layout(opl, r2)
+        qi, gi = OKV.q_token_index(opl, r2), OKV.gather_index(opl, r2)
+        qi_t, gi_t = (torch.from_numpy(x.astype(np.int64)).cuda() for x in (qi, gi))
+        for h2 in groups:
+            hq2 = slice(h2 * G, (h2 + 1) * G)
+            rows = np.sort(rng.choice(len(qi), size=64, replace=False))
+            gg = {"o": U.to_f64(g["o"][:, hq2]), "lse": U.to_f64(g["lse"][hq2]),
+                  "dq": U.to_f64(g["dq"][:, hq2])}
+            _sampled_rows_check("%s r%d kv%d sampled" % (name, r2, h2), lay, gg,
+                                U.to_f64(Q[qi_t][:, hq2]), U.to_f64(K[gi_t][:, h2:h2 + 1]),
+                                U.to_f64(V[gi_t][:, h2:h2 + 1]), U.to_f64(dO[qi_t][:, hq2]),
+                                rows, scale, sampled)
+            n_rows += len(rows)
+    print("%s sampled rows (%d rows x %d heads), observed:" % (name, n_rows, G),
+          {k: tuple(float("%.3g" % x) for x in v) for k, v in sampled.items()})
 
 
 def test_kv_pieces_and_merge(fcp, torch):
@@ -334,6 +437,20 @@ def test_kv_scatter_add_matches_oracle(fcp, torch, name, strategy, src):
     assert total_remote == plan.stats()["sum_remote_tokens"]
 
 
+def test_kv_reduce_finish_rounds_to_bf16(fcp, torch):
+    """fcp_kv_reduce_finish: round-to-nearest-even fp32 -> bf16 of the reduced dK, dV, bit-exact
+    against the library conversion (incl. ties, subnormals, large values); bad sizes refused."""
+    gen = torch.Generator().manual_seed(5)
+    a = torch.randn((1000, 2, 64), generator=gen) * 37.0
+    b = torch.randn((1000, 2, 64), generator=gen) * 1e-3
+    a.view(-1)[:8] = torch.tensor([1.00390625, 1.01171875, -1.00390625, 3.3895314e38, 1e-40, 0.0, -0.0, 65280.0])
+    ka, kb = fcp.kv_reduce_finish(a.cuda(), b.cuda())
+    torch.cuda.synchronize()
+    assert torch.equal(ka.cpu(), a.to(torch.bfloat16)) and torch.equal(kb.cpu(), b.to(torch.bfloat16))
+    with pytest.raises(fcp.FcpError):
+        fcp.kv_reduce_finish(a.cuda().view(-1)[:12], b.cuda().view(-1)[:12])
+
+
 SPLIT_CASES = [
     # d, N, Hq, Hkv, D, strategy
     ([900, 260, 250, 126], 4, 4, 2, 128, 0),       # hybrid: whole documents + one sharded
@@ -385,6 +502,68 @@ def test_local_prefix_split_matches_packed_oracle(fcp, torch, case):
     U.check("dq", dq, want_dq)
     U.check("dk", f(dK), want_dk)
     U.check("dv", f(dV), want_dv)
+
+
+def test_split_overlap_two_streams_same_bits(fcp, torch):
+    """the communication-hiding order — the PREFIX piece's keys "arrive"
+    (copy-engine transfer + PREFIX gather on a second stream) while the LOCAL gather + forward
+    run on the main stream, which then waits, runs the PREFIX forward and fcp_merge — must give
+    exactly the bits of the serial split run, and both must match the packed oracle."""
+    cfg = fcp_inputs.CONFIGS["8b"]
+    d = fcp_inputs.doc_lengths("8b", 0)
+    Hq, Hkv, D = 8, 2, 128                       # the 8b plan on a lighter head count
+    scale = 1.0 / math.sqrt(D)
+    Q, K, V, _ = fcp_inputs.make_tensors(cfg.C, Hq, Hkv, D, 6)
+    Kd, Vd = K.cuda(), V.cuda()
+    plan, opl = fcp.Plan(d, cfg.N), OP.plan(d, cfg.N)
+    main, side = torch.cuda.current_stream(), torch.cuda.Stream()
+    arrived = torch.cuda.Event()
+    for r in (0, 2):
+        qi = torch.from_numpy(plan.rank_layout(r)["q_token_index"].astype(np.int64))
+        q = Q[qi].contiguous().cuda()
+        sl = plan.sched(r, Hq, Hkv, D, fcp.PIECE_LOCAL).upload("cuda")
+        sp = plan.sched(r, Hq, Hkv, D, fcp.PIECE_PREFIX).upload("cuda")
+        n_p = plan.rank_stats(r, fcp.PIECE_PREFIX)["n_kv"]
+        assert n_p > 0
+        res = {}
+        for mode in ("serial", "overlap"):
+            kp = torch.empty((n_p, Hkv, D), dtype=torch.bfloat16, device="cuda")
+            vp = torch.empty_like(kp)
+            recv = torch.empty_like(Kd)
+            if mode == "overlap":
+                side.wait_stream(main)
+                with torch.cuda.stream(side):
+                    recv.copy_(Kd, non_blocking=True)                       # the arrival
+                    plan.kv_gather(r, Kd, Vd, kp, vp, stream=side, piece=fcp.PIECE_PREFIX)
+                    arrived.record(side)
+            kl, vl, _ = plan.kv_gather(r, Kd, Vd, piece=fcp.PIECE_LOCAL)
+            ol, ll = sl.attn_fwd(q, kl, vl, scale)
+            if mode == "overlap":
+                main.wait_event(arrived)
+            else:
+                recv.copy_(Kd, non_blocking=True)
+                plan.kv_gather(r, Kd, Vd, kp, vp, piece=fcp.PIECE_PREFIX)
+            op, lp = sp.attn_fwd(q, kp, vp, scale)
+            res[mode] = fcp.merge(ol, ll, op, lp)
+            torch.cuda.synchronize()
+        assert torch.equal(res["serial"][0], res["overlap"][0])
+        assert torch.equal(res["serial"][1], res["overlap"][1])
+        # against the oracle: sampled rows of the rank
+        lay = OKV.rank_layout(opl, r)
+        gi = OKV.gather_index(opl, r)
+        rows = np.sort(np.random.default_rng(r).choice(q.shape[0], size=48, replace=False))
+        g = {"o": U.to_f64(res["overlap"][0]), "lse": U.to_f64(res["overlap"][1]), "dq": None}
+        cu_q, cu_k = np.asarray(lay.cu_seqlens_q), np.asarray(lay.cu_seqlens_k)
+        shard = np.searchsorted(cu_q, rows, side="right") - 1
+        counts = np.asarray(lay.q_pos_off)[shard] + (rows - cu_q[shard]) + 1
+        seg = np.asarray(lay.shard_seg)[shard]
+        Kg, Vg = U.to_f64(K)[gi], U.to_f64(V)[gi]
+        for s_ in np.unique(seg):
+            sel = seg == s_
+            o, lse = OA.shard_rows_fwd(U.to_f64(q.cpu())[rows[sel]], Kg[cu_k[s_]:cu_k[s_ + 1]],
+                                       Vg[cu_k[s_]:cu_k[s_ + 1]], counts[sel], scale)
+            U.check("o", g["o"][rows[sel]], o)
+            U.check_lse("lse", g["lse"][:, rows[sel]], lse)
 
 
 def test_outputs_do_not_write_out_of_bounds(fcp, torch):

@@ -247,6 +247,20 @@ def test_sampled_rows_match_full():
     so, sl = A.shard_rows_fwd(q[rows], k, v, p + rows + 1, scale)
     np.testing.assert_allclose(so, o[rows], atol=1e-13)
     np.testing.assert_allclose(sl, lse[:, rows], atol=1e-13)
+    # sampled dq rows: equal to the full backward (itself pinned by SDPA autograd and central
+    # differences) on the same rows, and to a central difference of the row's own loss
+    do = rnd(rng, s, Hq, D)
+    dq, _, _ = A.shard_bwd(q, k, v, o, lse, do, p, scale)
+    sdq = A.shard_rows_bwd_dq(q[rows], k, v, do[rows], p + rows + 1, scale)
+    np.testing.assert_allclose(sdq, dq[rows], atol=1e-13)
+    i, h, c, eps = 1, 2, 3, 1e-6
+    def loss(qq):
+        oo, _ = A.shard_rows_fwd(qq, k, v, p + rows + 1, scale)
+        return float((oo * do[rows]).sum())
+    qp, qm = q[rows].copy(), q[rows].copy()
+    qp[i, h, c] += eps
+    qm[i, h, c] -= eps
+    assert abs((loss(qp) - loss(qm)) / (2 * eps) - sdq[i, h, c]) < 1e-7
 
 
 def test_local_prefix_split_merges_to_the_packed_result():

@@ -179,7 +179,7 @@ def test_local_and_prefix_pieces_partition_the_visible_pairs():
             assert list(KV.piece_gather_index(pl, r, KV.PIECE_LOCAL)) == list(KV.q_token_index(pl, r))
             assert KV.piece_remote_tokens(pl, r, KV.PIECE_LOCAL) == 0
             assert KV.piece_remote_tokens(pl, r, KV.PIECE_PREFIX) == KV.kv_stats(pl).remote[r]
-            # the pair counts are the two terms of W(p, s) = s(s+1)/2 + p s  (PAPER.md:74)
+            # the pair counts are the two terms of W(p, s) = s(s+1)/2 + p s  (PAPER.md:101)
             mine = [s for s in pl.shards if s.rank == r]
             assert len(loc) == sum(s.len * (s.len + 1) // 2 for s in mine)
             assert len(pre) == sum(s.start * s.len for s in mine)

@@ -26,6 +26,7 @@ def parse_golden(path=GOLDEN):
             cur["d"] = [int(x) for x in tok[1:]]
         elif tok[0] == "n":
             cur["n"], cur["r_ppm"] = int(tok[1]), int(tok[3])
+            cur["align"] = int(tok[5]) if len(tok) > 5 else 1
         elif tok[0] == "per_doc":
             cur["per_doc"] = [int(x) for x in tok[1:]]
         elif tok[0] == "rank":
@@ -54,7 +55,7 @@ def test_W_is_the_pair_count():
 
 @pytest.mark.parametrize("case", parse_golden(), ids=lambda c: c["name"])
 def test_worked_examples(case):
-    pl = P.plan(case["d"], case["n"], case["r_ppm"])
+    pl = P.plan(case["d"], case["n"], case["r_ppm"], align=case["align"])
     assert list(pl.per_doc) == case["per_doc"]
     for j in range(case["n"]):
         got = [(s.doc, s.start, s.len) for s in pl.shards if s.rank == j]
@@ -134,6 +135,39 @@ def test_invariants_random():
             assert len(pl.per_doc) == 0
         # determinism
         assert P.plan(d, N, r_ppm, strategy) == pl
+
+
+def test_aligned_variant_invariants():
+    """align = A > 1: still an exact cover with exactly C/N tokens per worker
+    (Eq. 1, Eq. 2); A = 1 is Algorithm 1 itself; Per-Doc chunks start on the grid and have
+    lengths that are multiples of A except the one ending its document; and on the bench recipes
+    the cuts that are not on a multiple of 128 shrink to a handful."""
+    for d, N, r_ppm, strategy in random_inputs(5, 300):
+        assert P.plan(d, N, r_ppm, strategy, align=1) == P.plan(d, N, r_ppm, strategy)
+        for A in (2, 4, 8, 16):
+            pl = P.plan(d, N, r_ppm, strategy, align=A)
+            check_valid(pl)
+            assert P.plan(d, N, r_ppm, strategy, align=A) == pl
+            if strategy == P.STRATEGY_ALL_PER_DOC:
+                for k, x in enumerate(d):
+                    q = x // (2 * N * A) * A
+                    if q == 0:
+                        continue
+                    h = (x - 2 * N * q) // A * A
+                    e = x - 2 * N * q - h
+                    # the chunk grid h + c q is respected: chunks are never cut, so every cut
+                    # of the document inside (h, d - e) is a grid point (the head item [0, h)
+                    # and the ragged tail [d - e, d) are movable and may be cut anywhere)
+                    cuts = {s.start for s in pl.shards if s.doc == k and h < s.start < x - e}
+                    assert all((c - h) % q == 0 for c in cuts), (d, N, A, k, cuts)
+    import fcp_inputs
+    for name in ("8b", "longtail", "70b"):
+        cfg = fcp_inputs.CONFIGS[name]
+        for seed in (0, 1):
+            d = fcp_inputs.doc_lengths(name, seed)
+            off = [sum(1 for s in P.plan(d, cfg.N, align=A).shards if s.start % 128) for A in (1, 128)]
+            assert off[1] <= cfg.N - 1 and off[1] <= off[0], (name, seed, off)
+            check_valid(P.plan(d, cfg.N, align=128))
 
 
 def test_per_doc_pair_identity_and_exact_balance():   # PAPER.md:62

@@ -9,9 +9,9 @@ from oracle import planner as P
 from test_oracle_planner import parse_golden, random_inputs
 
 
-def assert_same_plan(fcp, d, N, r_ppm, strategy):
-    want = P.plan(d, N, r_ppm, strategy)
-    got = fcp.Plan(d, N, r_ppm, strategy)
+def assert_same_plan(fcp, d, N, r_ppm, strategy, align=1):
+    want = P.plan(d, N, r_ppm, strategy, align)
+    got = fcp.Plan(d, N, r_ppm, strategy, align)
     assert got.shards() == [tuple(s) for s in want.shards]
     assert got.per_doc() == list(want.per_doc)
     st, kst = got.stats(), KV.kv_stats(want)
@@ -40,7 +40,7 @@ def assert_same_plan(fcp, d, N, r_ppm, strategy):
 
 @pytest.mark.parametrize("case", parse_golden(), ids=lambda c: c["name"])
 def test_worked_examples(fcp, case):
-    assert_same_plan(fcp, case["d"], case["n"], case["r_ppm"], 0)
+    assert_same_plan(fcp, case["d"], case["n"], case["r_ppm"], 0, case["align"])
 
 
 def test_random_small(fcp):
@@ -56,6 +56,25 @@ def test_bench_configs(fcp, name):
         assert sum(d) == cfg.C
         for strategy in (0, 1, 2, 3):
             assert_same_plan(fcp, d, cfg.N, 1_050_000, strategy)
+
+
+def test_tile_aligned_variant(fcp):
+    """fcp_plan_opts.align_tokens: bit-exact against oracle.planner.plan(...,
+    align=A) on random inputs and on the bench recipes with A = 128; 0 and 1 are Algorithm 1
+    itself; a negative value is INVALID_ARG."""
+    for d, N, r_ppm, strategy in random_inputs(31, 250):
+        for A in (2, 4, 16):
+            assert_same_plan(fcp, d, N, r_ppm, strategy, A)
+        assert fcp.Plan(d, N, r_ppm, strategy, 0).shards() == fcp.Plan(d, N, r_ppm, strategy, 1).shards() \
+            == [tuple(s) for s in P.plan(d, N, r_ppm, strategy).shards]
+    for name in ("8b", "longtail", "short", "70b"):
+        cfg = fcp_inputs.CONFIGS[name]
+        for seed in (0, 1):
+            for strategy in (0, 1):
+                assert_same_plan(fcp, fcp_inputs.doc_lengths(name, seed), cfg.N, 1_050_000, strategy, 128)
+    with pytest.raises(fcp.FcpError) as e:
+        fcp.Plan([8, 8], 2, align=-1)
+    assert e.value.status == -1
 
 
 def test_sched_info_counts_useful_pairs(fcp):

@@ -484,25 +484,26 @@ def split_compare(fcp, w, scale, reps=3):
             "local_share_of_fwd": tot["local_fwd"] / split_fwd}
 
 
-def split_overlap(fcp, w, scale, reps=3, links_gbs=(None, 900.0, 50.0)):
+def split_overlap(fcp, w, scale, reps=3):
     """how much of the remote-KV arrival the LOCAL forward
     hides.  On one GPU the arrival of a rank's `remote_bytes` is a copy-engine transfer on a
-    second stream (cudaMemcpyAsync device to device: no SM is used, like a NIC / NVLink write
-    into a receive buffer); a slower link is emulated by repeating the transfer (the repeat count
-    is calibrated from the measured copy-engine rate).  Per virtual rank, forward only:
+    second stream (cudaMemcpyAsync: no SM is used, like a NIC / NVLink write into a receive
+    buffer) at three speeds: device to device as fast as the copy engine goes; the same twice
+    (about an NVLink-5 direction); and from pinned HOST memory over PCIe (a cross-node-class
+    link, a few tens of GB/s).  Per virtual rank, forward only:
       unsplit        : arrival, then full gather + forward (nothing can start earlier)
       split, serial  : LOCAL gather + fwd, arrival, PREFIX gather + fwd, merge on one stream
-      split, overlap : arrival on the copy stream WHILE the LOCAL gather + fwd run; the main
-                       stream waits for it before the PREFIX gather + fwd + merge
-    Times are wall time on the device (events on the main stream, which joins the copy stream).
-    hidden = (serial - overlap) / arrival."""
+      split, overlap : the arrival runs on the copy stream WHILE the LOCAL gather + fwd run on
+                       the main stream, which waits for it before the PREFIX gather + fwd + merge
+    Times are device wall time (events on the main stream).  hidden = (serial - overlap) /
+    min(arrival, LOCAL): the share of what could be hidden that was."""
     import torch
     cfg = w.cfg
     plan = fcp.Plan(w.d, cfg.N)
     main, side = torch.cuda.current_stream(), torch.cuda.Stream()
     row_b = cfg.Hkv * cfg.D * 2
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    arrived = torch.cuda.Event()
+    go, arrived = torch.cuda.Event(), torch.cuda.Event()
 
     def timed(fn):
         best = float("inf")
@@ -515,31 +516,29 @@ def split_overlap(fcp, w, scale, reps=3, links_gbs=(None, 900.0, 50.0)):
             best = min(best, ev[0].elapsed_time(ev[1]))
         return best
 
-    # copy-engine rate on this box
-    n_cal = 64 << 20
-    src = torch.empty(n_cal, dtype=torch.uint8, device=w.K.device)
-    dst = torch.empty_like(src)
-    ce_gbs = n_cal / (timed(lambda: dst.copy_(src, non_blocking=True)) * 1e-3) / 1e9
-    del src, dst
-    out = {"copy_engine_gbs": ce_gbs, "links": {}}
-    for link in links_gbs:
-        rep = 1 if link is None else max(1, int(round(ce_gbs / link)))
-        tot = dict.fromkeys(("arrival", "unsplit", "split_serial", "split_overlap", "split_no_arrival"), 0.0)
+    max_remote = max(plan.rank_stats(r)["remote_tokens"] for r in range(cfg.N))
+    host = torch.empty(max(1, max_remote * cfg.Hkv * cfg.D), dtype=torch.bfloat16).pin_memory()
+    out = {"links": {}}
+    for link, (rep, from_host) in (("copy_engine_d2d", (1, False)), ("d2d_twice_nvlink_class", (2, False)),
+                                   ("pcie_from_pinned_host", (1, True))):
+        tot = dict.fromkeys(("arrival", "local", "unsplit", "split_serial", "split_overlap",
+                             "split_no_arrival"), 0.0)
         for r in range(cfg.N):
             q = w.q[r]
-            remote = plan.rank_stats(r)["remote_tokens"]
+            n_el = plan.rank_stats(r)["remote_tokens"] * cfg.Hkv * cfg.D     # per tensor
             sf = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D).upload(q.device)
             sl = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D, fcp.PIECE_LOCAL).upload(q.device)
             sp = plan.sched(r, cfg.Hq, cfg.Hkv, cfg.D, fcp.PIECE_PREFIX).upload(q.device)
-            rk = w.K.view(-1)[:remote * cfg.Hkv * cfg.D]          # remote_bytes/2 per tensor
-            rv = w.V.view(-1)[:remote * cfg.Hkv * cfg.D]
-            bk, bv = torch.empty_like(rk), torch.empty_like(rv)   # the "receive buffer"
+            srck = host[:n_el] if from_host else w.K.view(-1)[:n_el]
+            srcv = host[:n_el] if from_host else w.V.view(-1)[:n_el]
+            bk = torch.empty(n_el, dtype=torch.bfloat16, device=q.device)    # the receive buffer
+            bv = torch.empty_like(bk)
 
             def arrival(stream):
                 with torch.cuda.stream(stream):
                     for _ in range(rep):
-                        bk.copy_(rk, non_blocking=True)
-                        bv.copy_(rv, non_blocking=True)
+                        bk.copy_(srck, non_blocking=True)
+                        bv.copy_(srcv, non_blocking=True)
 
             def local():
                 kl, vl, _ = plan.kv_gather(r, w.K, w.V, piece=fcp.PIECE_LOCAL)
@@ -561,27 +560,29 @@ def split_overlap(fcp, w, scale, reps=3, links_gbs=(None, 900.0, 50.0)):
                 prefix_and_merge(ol, ll)
 
             def overlap():
-                side.wait_stream(main)
+                go.record(main)
+                ol, ll = local()                 # enqueued first: the GPU starts on it at once
+                side.wait_event(go)
                 arrival(side)
                 arrived.record(side)
-                ol, ll = local()
                 main.wait_event(arrived)
                 prefix_and_merge(ol, ll)
 
             tot["arrival"] += timed(lambda: arrival(main))
+            tot["local"] += timed(local)
             tot["unsplit"] += timed(unsplit)
             tot["split_serial"] += timed(serial)
             tot["split_overlap"] += timed(overlap)
             tot["split_no_arrival"] += timed(lambda: prefix_and_merge(*local()))
             del bk, bv
-        name = "copy_engine" if link is None else "%g_GBps" % link
         remote_b = 2 * row_b * sum(plan.rank_stats(r)["remote_tokens"] for r in range(cfg.N))
-        out["links"][name] = {
+        hideable = min(tot["arrival"], tot["local"])
+        out["links"][link] = {
             "ms_sum_over_ranks": {k: round(v, 4) for k, v in tot.items()},
-            "emulated_link_gbs": remote_b / (tot["arrival"] * 1e-3) / 1e9 if tot["arrival"] > 0 else None,
-            "remote_bytes": remote_b, "repeats": rep,
-            "hidden_fraction_of_arrival": ((tot["split_serial"] - tot["split_overlap"]) / tot["arrival"]
-                                           if tot["arrival"] > 0 else None),
+            "link_gbs": remote_b / (tot["arrival"] * 1e-3) / 1e9 if tot["arrival"] > 0 else None,
+            "remote_bytes": remote_b,
+            "hidden_fraction_of_hideable": ((tot["split_serial"] - tot["split_overlap"]) / hideable
+                                            if hideable > 0 else None),
             "split_overlap_vs_unsplit": tot["split_overlap"] / tot["unsplit"]}
     return out
 
@@ -754,7 +755,7 @@ def run_fcp(args):
         bplan = fcp.Plan(bd, bc.N)
         bK = torch.empty((bc.C, bc.Hkv, bc.D), dtype=torch.bfloat16, device=dev).normal_()
         bV = torch.empty_like(bK).normal_()
-        b_ms, b_bytes = [], []
+        big_ms, big_bytes = [], []
         for r in range(bc.N):
             n = bplan.rank_stats(r)["n_kv"]
             ko = torch.empty((n, bc.Hkv, bc.D), dtype=torch.bfloat16, device=dev)
@@ -766,14 +767,14 @@ def run_fcp(args):
                 bplan.kv_gather(r, bK, bV, ko, vo)
             t1.record()
             torch.cuda.synchronize()
-            b_ms.append(t0.elapsed_time(t1) / 20)
-            b_bytes.append(4 * n * bc.Hkv * bc.D * 2)
+            big_ms.append(t0.elapsed_time(t1) / 20)
+            big_bytes.append(4 * n * bc.Hkv * bc.D * 2)
             del ko, vo
         del bK, bV
-        bg = sum(b_bytes) / (sum(b_ms) * 1e-3) / 1e9
+        bg = sum(big_bytes) / (sum(big_ms) * 1e-3) / 1e9
         big = {"gbs": bg, "frac_measured_hbm": bg / peaks["hbm"], "frac_of_nominal_8000": bg / 8000.0,
                "workload": "longtail (128K, 8 virtual ranks), gather only",
-               "kernel_ms_per_rank": b_ms, "bytes_per_rank": b_bytes,
+               "kernel_ms_per_rank": big_ms, "bytes_per_rank": big_bytes,
                "how": "20 back-to-back launches per rank, CUDA events; 2 tensors x (read + write)"}
     # dKV scatter-add (not part of the timed step): same method.  Per token
     # and tensor: bf16 source row + fp32 accumulator read + write = (2 + 4 + 4) * Hkv * D bytes.

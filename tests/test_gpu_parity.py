@@ -154,11 +154,13 @@ def test_key_count_closed_form_full_size(fcp, torch, name, ranks):
         del q, kg, vg, o, lse
 
 
-# (max-abs, mean-abs) bounds of test_forward_running_max_growth; PLACEHOLDER = the round-1 bounds
-# until the observed errors are in (see the test)
+# (max-abs, mean-abs) bounds of test_forward_running_max_growth = about twice the errors observed
+# on B200 (round 2: D=128 dq 0.593 / 0.0178, dk 3.3e-3, dv 0.034 at |dv| <= 14.9, lse 1.2e-4;
+# D=64 dq 0.406 / 0.0162, dk 9.6e-3, dv 0.044 at |dv| <= 12.9, lse 1.2e-4; max|K| 187 / 174).
+# dk keeps the plain north-star bound, dv gets 3e-2 plus the bf16 half-ulp of DESIGN.md section 8.
 GROWTH_BOUNDS = {
-    128: {"dq": (2e-2 + 5e-3 * 190, 2e-3 + 2e-4 * 190), "dk": (5e-2, 5e-3), "dv": (5e-2, 5e-3)},
-    64: {"dq": (2e-2 + 5e-3 * 190, 2e-3 + 2e-4 * 190), "dk": (5e-2, 5e-3), "dv": (5e-2, 5e-3)},
+    128: {"dq": (1.2, 3.6e-2), "dk": (2e-2, 2e-3), "dv": (3e-2, 2e-3)},
+    64: {"dq": (0.8, 3.3e-2), "dk": (2e-2, 2e-3), "dv": (3e-2, 2e-3)},
 }
 
 
@@ -189,12 +191,13 @@ def test_forward_running_max_growth(fcp, torch, D, Hq, Hkv):
     assert float(np.max(w["lse"])) > 40.0           # the case really is steep
     U.check("o", U.to_f64(g["o"]), w["o"])
     lse_g = U.to_f64(g["lse"])
-    assert np.abs(lse_g - w["lse"]).max() <= 1e-3 * max(1.0, float(np.abs(w["lse"]).max()) / 8.0)
+    assert np.abs(lse_g - w["lse"]).max() <= U.TOL_LSE
     # dq = scale * dS K with |K| up to ~190 here.  The rows of dS sum to zero and K varies slowly
     # along the keys, so dq (a few units) is what is left of terms ~|dS| |K| cancelling; the bf16
     # rounding of dS (2^-9 relative, sum_j |dS_ij| ~ 10-20) breaks the cancellation by about
-    # scale * 2^-9 * 20 * max|K| ~ 3.5e-3 * max|K|.  The north_star tolerance (stated for N(0,1)
-    # inputs, max|K| ~ 4) is widened by that term.
+    # scale * 2^-9 * 20 * max|K| ~ 3.5e-3 * max|K| ~ 0.6 — which is what is observed.  The
+    # north_star tolerance is stated for N(0,1) inputs (max|K| ~ 4); here the bound is twice the
+    # observed error (GROWTH_BOUNDS).
     kmax = float(K.abs().max())
     obs = {k: (float(np.abs(U.to_f64(g[k]) - w[k]).max()), float(np.abs(U.to_f64(g[k]) - w[k]).mean()),
                float(np.abs(w[k]).max())) for k in ("dq", "dk", "dv")}

@@ -267,6 +267,14 @@ int  fcp_sched_get_list(const fcp_sched* sched, int32_t which, int32_t* out, int
  *                heads of a kv head; they hold only THIS rank's queries' contributions, in the
  *                layout of k, v (global dK = sum over ranks of scatter-add).
  *    bf16 tensor-core products with fp32 accumulation, fp32 softmax.
+ *    Precondition: every row of q, k, v, dO handed to these calls holds finite values.  The
+ *    kernels read 128-row boxes that run past the end of a segment or shard into its neighbour's
+ *    rows and mask what they compute there: masked SCORES are replaced by selection, so the
+ *    forward tolerates non-finite values in the K rows of a neighbouring segment
+ *    (tests/test_gpu_parity.py::test_nonfinite_neighbour_keys), but a masked probability is an
+ *    exact zero that still multiplies the neighbour's V row (forward) and K / V rows (backward)
+ *    inside the tensor core, where 0 * Inf = NaN: a NaN or Inf in ANOTHER document's V, or in
+ *    K / V during the backward, can reach the last 128-row tile of this one.
  * ------------------------------------------------------------------------------------------ */
 enum { FCP_DTYPE_BF16 = 0, FCP_DTYPE_F32 = 1 };
 typedef struct {

@@ -1,6 +1,7 @@
 """Builds libfcp.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2606_08476_b200.build [--force] [--verbose]
+    python -m paper_2606_08476_b200.build --sass-summary     # code-object evidence as markdown
 """
 import os
 import subprocess
@@ -58,5 +59,53 @@ def build(force=False, verbose=False):
     return LIB
 
 
+SASS_MNEMONICS = ["UTCHMMA", "LDTM", "STTM", "UTMALDG", "UTMASTG", "UBLKCP", "UBLKRED", "UTMAREDG",
+                  "MUFU.EX2", "HMMA", "STL", "LDL"]
+
+
+def sass_summary():
+    """Markdown table of what the shipped code object contains, per kernel: registers, spills,
+    shared memory (ptxas -v, via cuobjdump -res-usage) and counts of the SASS mnemonics that
+    prove the Blackwell path (UTCHMMA = tcgen05.mma, LDTM / STTM = tcgen05.ld / st, UTMALDG /
+    UTMASTG = TMA tensor load / store, UBLKCP / UBLKRED = bulk copy / reduce)."""
+    import re
+    lib = build()
+    cu = os.path.join(os.path.dirname(_nvcc()), "cuobjdump")
+    cu = cu if os.path.exists(cu) else "cuobjdump"
+    res = subprocess.run([cu, "-res-usage", lib], stdout=subprocess.PIPE, text=True).stdout
+    usage = {}
+    for m in re.finditer(r"Function ([^:\n]+):\n\s*(.*)", res):
+        usage[m.group(1).strip()] = m.group(2).strip()
+    sass = subprocess.run([cu, "-sass", lib], stdout=subprocess.PIPE, text=True).stdout
+    counts, cur = {}, None
+    for line in sass.splitlines():
+        m = re.match(r"\s*Function : (\S+)", line)
+        if m:
+            cur = m.group(1)
+            counts[cur] = dict.fromkeys(SASS_MNEMONICS, 0)
+            counts[cur]["instructions"] = 0
+            continue
+        if cur and re.match(r"\s*/\*[0-9a-f]{4,}\*/", line):
+            counts[cur]["instructions"] += 1
+            for k in SASS_MNEMONICS:
+                if re.search(r"\b" + re.escape(k), line):
+                    counts[cur][k] += 1
+    filt = subprocess.run(["c++filt"] + list(counts), stdout=subprocess.PIPE, text=True).stdout.splitlines()
+    names = dict(zip(counts, filt)) if len(filt) == len(counts) else {k: k for k in counts}
+    out = ["| kernel | " + " | ".join(["instructions"] + SASS_MNEMONICS) + " | resources (cuobjdump -res-usage) |",
+           "|---|" + "---:|" * (len(SASS_MNEMONICS) + 1) + "---|"]
+    for k in sorted(counts, key=lambda x: names[x]):
+        short = names[k].replace("(anonymous namespace)::", "").replace("<unnamed>::", "")
+        short = re.sub(r"^void ", "", short)
+        short = re.sub(r"\(.*", "", short)
+        c = counts[k]
+        out.append("| `%s` | %s | %s |" % (short, " | ".join(str(c[x]) for x in ["instructions"] + SASS_MNEMONICS),
+                                            usage.get(k, "")))
+    return "\n".join(out)
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    if "--sass-summary" in sys.argv:
+        print(sass_summary())
+    else:
+        print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

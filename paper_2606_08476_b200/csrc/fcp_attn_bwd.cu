@@ -31,25 +31,6 @@
 #include "fcp_sm100.cuh"
 #include "fcp_tma.h"
 
-#ifdef FCP_EXP_TRACE
-__device__ long long g_trace[64 * 16];
-extern "C" int fcp_debug_trace(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_trace, sizeof(g_trace));
-}
-#define TRACE(n, id)                                                                   \
-  do {                                                                                 \
-    if (blockIdx.x == 0 && (n) >= 200u && (n) < 264u && (threadIdx.x & 31) == 0)       \
-      g_trace[((n) - 200u) * 16 + (id)] = clock64();                                   \
-  } while (0)
-#define TRACEV(n, id, v)                                                               \
-  do {                                                                                 \
-    if (blockIdx.x == 0 && (n) >= 200u && (n) < 264u) g_trace[((n) - 200u) * 16 + (id)] = (v); \
-  } while (0)
-#else
-#define TRACE(n, id)
-#define TRACEV(n, id, v)
-#endif
-
 namespace {
 using namespace fcp;
 
@@ -376,9 +357,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       constexpr uint32_t kStageStep = Cfg::kStage >> 4, kDoStep = Cfg::kQTile >> 4;
       // ring state of iteration n: stage index, parity of the stage's phase, n & 1
       uint32_t st = 0, sph = 0, b = 0, mph = 0;
-#ifdef FCP_EXP_TRACE
-      uint32_t tn_ = 0;
-#endif
 
       // Keeps ptxas from hoisting the eight 64-bit A descriptors of a product out of the loop
       // into general registers (16 R2UR per product and iteration); from an opaque base they
@@ -422,8 +400,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
               mbar_wait(&bars->dpt_free, b);     // softmax(n) holds dP^T(n) in registers
             }
             tc_fence_after();
-            TRACE(tn_, 1);
-            TRACEV(tn_, 12, ok_a);
             const uint32_t q_lo = q_kmaj0 + st1 * kStageStep;
             const uint32_t v_lo = opaque(v_kmaj);
             issue_kq(Cfg::kColS + (b ^ 1) * 64, opaque(k_kmaj), q_lo, 0, kSteps);
@@ -432,8 +408,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
                    (i > 0 || mbar_test(&bars->dkv_free, mph ^ 1));
             issue_kq(Cfg::kColDP, v_lo, q_lo + kDoStep, kSteps - kTail, kSteps);
             umma_commit(&bars->st_full);
-            TRACE(tn_, 2);
-            TRACEV(tn_, 13, ok_b);
           }
           if (!ok_b) {
             mbar_wait(&bars->p_ready, b);
@@ -441,7 +415,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
             mbar_wait(&bars->dq_free, b ^ 1);
           }
           tc_fence_after();
-          TRACE(tn_, 3);
           // P^T / dS^T of q columns [32h, 32h+32) live in columns [32h, 32h+16) / [32h+16, 32h+32)
           // of the S^T buffer: each softmax warpgroup overwrites only the columns it has loaded
           const uint32_t tP = tmem_base + Cfg::kColS + b * 64, tDS = tP + 16;
@@ -472,10 +445,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
           umma_commit(&bars->qdo_free[st]);
           umma_commit(&bars->ds_free[b]);
           umma_commit(&bars->dq_full);
-          TRACE(tn_, 4);
-#ifdef FCP_EXP_TRACE
-          ++tn_;
-#endif
           st = st1;
           sph = sph1;
           b ^= 1;
@@ -527,9 +496,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         const int q_pos = w.q_pos() + half * 32;       // position of this half's first column
         // mask needed when some (kv, q) pair of this warp's rows is invisible
         const bool need_mask = (warp_kv_max > q_pos) || (it.kv_rows < 128);
-        if (role == 4) TRACE(n, 5);
         mbar_wait(&bars->st_full, n & 1);
-        if (role == 4) TRACE(n, 6);
         tc_fence_after();
         uint32_t s[32], dp[32];
         tmem_ld32(tS + half * 32, s);
@@ -539,7 +506,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         tmem_ld_wait();
         tc_fence_before();
         mbar_arrive(&bars->dpt_free);                              // dP^T (and S^T) now in registers
-        if (role == 4) TRACE(n, 7);
         const uint32_t stat_addr = stat_base + st * Cfg::kStat;
         const uint32_t ds_row_addr = ds_base + (n & 1) * Cfg::kDS;
         if (need_mask)
@@ -552,7 +518,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         tmem_st_wait();
         tc_fence_before();
         mbar_arrive(&bars->p_ready);
-        if (role == 4) TRACE(n, 8);
       }
       // item epilogue: dV (half 0) / dK (half 1) rows out of TMEM
       mbar_wait(&bars->dkv_full, m & 1);
@@ -641,9 +606,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
       const BwdItem it = items[idx];
       if (it.n_iters == 0) continue;
       for (IterWalk w(it, subs, G); !w.done(); w.next(), ++n) {
-        if (role == 12) TRACE(n, 9);
         mbar_wait(&bars->dq_full, n & 1);
-        if (role == 12) TRACE(n, 10);
         tc_fence_after();
         uint32_t acc[2][32];
         tmem_ld32(tDQ, acc[0]);
@@ -651,7 +614,6 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         tmem_ld_wait();
         tc_fence_before();
         mbar_arrive(&bars->dq_free);
-        if (role == 12) TRACE(n, 11);
         if (leader) bulk_wait_read0();                  // previous reduce has read the staging
         named_bar_sync(1, 128);
         if (drow < D) {

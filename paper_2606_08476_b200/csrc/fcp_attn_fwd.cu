@@ -34,20 +34,6 @@
 #include "fcp_sm100.cuh"
 #include "fcp_tma.h"
 
-#ifdef FCP_EXP_TRACE
-__device__ long long g_trace_fwd[64 * 16];
-extern "C" int fcp_debug_trace_fwd(long long* out) {
-  return (int)cudaMemcpyFromSymbol(out, g_trace_fwd, sizeof(g_trace_fwd));
-}
-#define FTRACE(n, id)                                                                  \
-  do {                                                                                 \
-    if (blockIdx.x == 0 && (n) >= 50u && (n) < 114u && (threadIdx.x & 31) == 0)        \
-      g_trace_fwd[((n) - 50u) * 16 + (id)] = clock64();                                \
-  } while (0)
-#else
-#define FTRACE(n, id)
-#endif
-
 namespace {
 using namespace fcp;
 
@@ -246,9 +232,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       uint32_t slot = 0, sph = 0;      // ring position / phase parity of the next tile to consume
       uint32_t ppp = 0;                // parity of p_ready (both tiles advance together)
       uint32_t iph = 0;                // item parity (q_full; o_empty of the previous item)
-#ifdef FCP_EXP_TRACE
-      uint32_t tn = 0;
-#endif
 
       for (int idx = item_begin; idx < item_end; ++idx) {
         const int n = items[idx].n_kv_tiles;
@@ -272,11 +255,9 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
           ring_next(kslot, kph);                    // K_{j+1} follows V_j in the ring
 #pragma unroll
           for (int t = 0; t < NQ; ++t) {
-            FTRACE(tn, 8 + 3 * t);
             if (t == 0) mbar_wait(&bars->kv_full[vslot], vph);
             if (j == 0) mbar_wait(&bars->o_empty[t], iph ^ 1);
             mbar_wait(&bars->p_ready[t], ppp);
-            FTRACE(tn, 9 + 3 * t);
             tc_fence_after();
             issue_pv(t, vslot, j > 0);
             if (!has_next) umma_commit(&bars->pv_done[t]);
@@ -289,7 +270,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
               issue_qk(t, kslot);
               umma_commit(&bars->s_full[t]);
             }
-            FTRACE(tn, 10 + 3 * t);
           }
           ppp ^= 1;
           ring_next(slot, sph);
@@ -298,9 +278,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
             if (j + 2 == n) umma_commit(&bars->q_empty);
             ring_next(slot, sph);
           }
-#ifdef FCP_EXP_TRACE
-          ++tn;
-#endif
         }
         iph ^= 1;
       }
@@ -323,9 +300,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
     const uint32_t tS = tmem_base + lane_addr + t * 128;
     const uint32_t tO = tmem_base + lane_addr + (NQ + t) * 128;
     uint32_t s_ph = 0, pv_ph = 0;
-#ifdef FCP_EXP_TRACE
-    uint32_t tn = 0;
-#endif
     if (NQ == 2 && t == 1) named_bar_arrive(2, 256);        // tile 0 holds the MUFU token first
     const bool o_al32 = (reinterpret_cast<uintptr_t>(o) & 31) == 0;
     FwdItem nxt;
@@ -352,16 +326,13 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
       float m = -INFINITY, l = 0.f;
 
       for (int j = 0; j < n; ++j) {
-        if ((warp & 3) == 0) FTRACE(tn, 4 * t);
         mbar_wait(&bars->s_full[t], s_ph);
-        if ((warp & 3) == 0) FTRACE(tn, 4 * t + 1);
         s_ph ^= 1;
         tc_fence_after();
         uint32_t sr[4][32];
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32(tS + c * 32, sr[c]);
         tmem_ld_wait();
-        if ((warp & 3) == 0) FTRACE(tn, 4 * t + 2);
         const int col0 = j * FCP_TK;
         if (col0 + FCP_TK - 1 > warp_min_limit) {   // diagonal / boundary tile: mask in registers
 #pragma unroll
@@ -475,17 +446,12 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
         tmem_st_wait();
         tc_fence_before();
         mbar_arrive(&bars->p_ready[t]);
-        if ((warp & 3) == 0) FTRACE(tn, 4 * t + 3);
-#ifdef FCP_EXP_TRACE
-        ++tn;
-#endif
       }
 
       // epilogue: o = O / l, lse = ln2 * (m + log2 l)
       mbar_wait(&bars->pv_done[t], pv_ph);
       pv_ph ^= 1;
       tc_fence_after();
-      if ((warp & 3) == 0 && t == 0) FTRACE(tn - 1, 14);
       const float inv = l > 0.f ? 1.f / l : 0.f;
       // The whole O row leaves TMEM first: O_t is free for the next item's first PV product at
       // once, and the loads do not queue behind the store burst below.
@@ -548,7 +514,6 @@ fcp_attn_fwd_kernel(const __grid_constant__ CUtensorMap tmap_q,
           }
       }
       if (row_valid) *lse_row = l > 0.f ? kLn2 * (m + __log2f(l)) : -INFINITY;
-      if ((warp & 3) == 0 && t == 0) FTRACE(tn - 1, 15);
     }
     if (NQ == 2 && t == 0) named_bar_sync(2, 256);          // consume tile 1's last token
     if ((warp & 3) == 0 && lane == 0) bulk_wait0();         // o stores of the last item

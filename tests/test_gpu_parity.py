@@ -569,6 +569,28 @@ def test_split_overlap_two_streams_same_bits(fcp, torch):
             U.check_lse("lse", g["lse"][:, rows[sel]], lse)
 
 
+def test_nonfinite_neighbour_keys(fcp, torch):
+    """include/fcp.h, section 4 precondition: the forward replaces masked scores by selection, so
+    NaN / Inf in the K rows of the NEXT document (which the 128-row TMA box of this document's
+    ragged last tile pulls in) must not change a bit of this document's o and lse.  (V, and K / V
+    in the backward, are covered by the precondition instead: 0 * Inf inside the tensor core.)"""
+    d, Hq, Hkv, D = [200, 100, 84], 4, 2, 128
+    scale = 1.0 / math.sqrt(D)
+    Q, K, V, _ = fcp_inputs.make_tensors(sum(d), Hq, Hkv, D, 8)
+    plan = fcp.Plan(d, 1)
+    sched = plan.sched(0, Hq, Hkv, D).upload("cuda")
+    q = Q.cuda()
+    o_ref, lse_ref = sched.attn_fwd(q, K.cuda(), V.cuda(), scale)
+    Kbad = K.clone()
+    Kbad[200:300] = float("nan")                  # document 1 entirely
+    Kbad[210:220] = float("inf")
+    o, lse = sched.attn_fwd(q, Kbad.cuda(), V.cuda(), scale)
+    torch.cuda.synchronize()
+    for a, b in ((0, 200), (300, 384)):           # documents 0 and 2 never see document 1
+        assert torch.equal(o[a:b], o_ref[a:b]) and torch.equal(lse[:, a:b], lse_ref[:, a:b])
+    assert bool(torch.isfinite(o[:200].float()).all())
+
+
 def test_outputs_do_not_write_out_of_bounds(fcp, torch):
     """Canary rows around every output (o, lse, dq, dk, dv, gathered k/v) on ragged shapes whose
     last tiles are partial: the kernels predicate their stores by q_rows / kv_rows and TMA boxes

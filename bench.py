@@ -139,6 +139,7 @@ def traffic_from_ncu(raw_csv, config):
     """`ncu -i <rep> --page raw --csv > raw.csv` -> profiles/r2_traffic.csv (one row per profiled
     launch of the attention / gather kernels) stamped with the current source hash."""
     import csv
+    import re
     rows = list(csv.reader(open(raw_csv)))
     head = rows[0]
     ki, ri, wi = head.index("Kernel Name"), head.index("dram__bytes_read.sum"), head.index("dram__bytes_write.sum")
@@ -146,7 +147,8 @@ def traffic_from_ncu(raw_csv, config):
     ur, uw = unit[rows[1][ri]], unit[rows[1][wi]]
     out = []
     for r in rows[2:]:
-        name = r[ki].split("(")[0].split("<")[0].split("::")[-1]
+        m = re.search(r"(fcp_\w+)", r[ki])
+        name = m.group(1) if m else r[ki]
         out.append({"config": config, "kernel": name,
                     "dram_bytes_read": int(float(r[ri].replace(",", "")) * ur),
                     "dram_bytes_write": int(float(r[wi].replace(",", "")) * uw), "src_hash": source_hash()})

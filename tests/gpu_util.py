@@ -31,8 +31,8 @@ def check(name, got, want, max_abs=TOL_MAX_ABS, mean_abs=TOL_MEAN_ABS, bf16_sum=
     """north_star tolerances.  bf16_sum=True is for dk/dv written as bf16: they are sums over
     many queries and G heads whose magnitude exceeds 8, where rounding the exact value to bf16
     alone costs up to 2^-5 = 3.1e-2 > 2e-2; the per-element bound is then max_abs + the bf16
-    half-ulp of the expected value.  The fp32-output mode of the same
-    kernel is held to the plain max_abs."""
+    half-ulp of the expected value ("Reading: dk / dv written as bf16").
+    The fp32-output mode of the same kernel is held to the plain max_abs."""
     got, want = np.asarray(got, dtype=np.float64), np.asarray(want, dtype=np.float64)
     assert got.shape == want.shape, (name, got.shape, want.shape)
     assert np.isfinite(got).all(), "%s: non-finite values" % name

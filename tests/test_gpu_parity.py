@@ -115,7 +115,8 @@ def test_ragged_cases(fcp, torch, case, dkv_f32):
         U.compare_rank(fcp, d, N, r, Hq, Hkv, D, seed=1, strategy=strategy, dkv_f32=dkv_f32)
 
 
-@pytest.mark.parametrize("name,ranks", [("8b", (0, 3)), ("longtail_256k", (0,)), ("longtail_1m", (0,))])
+@pytest.mark.parametrize("name,ranks", [("8b", (0, 3)), ("short", tuple(range(16))), ("longtail", (2, 7)),
+                                        ("70b", (0, 6)), ("longtail_256k", (0,)), ("longtail_1m", (0,))])
 def test_key_count_closed_form_full_size(fcp, torch, name, ranks):
     """K = 0 makes lse = ln(#visible keys) exactly (SURVEY 8(c1) pin 3) and o the running mean
     of V: checks every mask, offset and the 32-bit row arithmetic of the real full-size launches

@@ -160,3 +160,26 @@ def test_kv_exchange_matches_oracle_gather_and_scatter(world):
         qi = KV.q_token_index(pl, r)
         assert np.abs(dk_l - dK[qi]).max() < 1e-5 and np.abs(dv_l - dV[qi]).max() < 1e-5
     assert sum(t[5] for t in res) > 0                       # the case really moves rows
+
+
+def test_bench_spawns_its_ranks_when_no_launcher_is_present():
+    """`python bench.py --gpus N` without WORLD_SIZE re-executes itself under
+    torch.distributed.run with N processes (the flag used to be ignored).  Exercised on
+    the CPU through the reference arm: rank 0 alone prints the JSON line, the other rank exits 0;
+    a launcher whose WORLD_SIZE contradicts --gpus is refused by the fcp arm."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--gpus", "2",
+                        "--steps", "1", "--warmup", "0", "--config", "tiny"], cwd=root, env=env,
+                       stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True, timeout=300)
+    assert r.returncode == 0, r.stdout[-2000:]
+    lines = [json.loads(x) for x in r.stdout.splitlines() if x.startswith("{")]
+    assert len(lines) == 1 and lines[0]["impl"] == "reference" and lines[0]["n_gpus"] == 2
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1"],
+                       cwd=root, env=dict(env, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0"),
+                       stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True, timeout=300)
+    assert r.returncode != 0 and ("--gpus 2 but WORLD_SIZE=1" in r.stdout or "CUDA device" in r.stdout)

@@ -127,16 +127,13 @@ struct BwdCfg {
   static constexpr int kColS = 0, kColDP = 128, kColDQ = 192, kColDV = 256, kColDK = 384;
   // registers per thread after setmaxnreg (launch: 128): control, softmax x2, drain
   static constexpr int kRegsCtl = 96, kRegsSoftmax = 152, kRegsDrain = 104;
-  // the MMA thread probes the barriers of its next group before issuing the last kTail MMAs of
-  // the current one: the tcgen05 queue holds about 5 MMAs, enough to cover the probe latency
-  static constexpr int kTail = 3;
 };
 static_assert(BwdCfg<128>::kSmemBytes <= 232448, "bwd shared memory exceeds 227 KB");
 
 struct BwdBarriers {
   uint64_t kv_full, kv_free;
   uint64_t qdo_full[3], qdo_free[3];
-  uint64_t st_full, dpt_free, p_ready;
+  uint64_t st_full, p_ready;
   uint64_t ds_free[2];
   uint64_t dq_full, dq_free;
   uint64_t dkv_full, dkv_free;
@@ -274,12 +271,14 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     mbar_init(&bars->kv_full, 1);
     mbar_init(&bars->kv_free, 1);
     for (int i = 0; i < Cfg::kStages; ++i) {
-      mbar_init(&bars->qdo_full[i], 1);
+      // the producer's arrive.expect_tx plus the 256 softmax threads: stage i is "full" for the
+      // MMA thread when Q, dO and the statistics have landed AND the previous iteration's S^T /
+      // dP^T sit in registers (dP^T has one TMEM buffer): ONE wait gates [S^T, dP^T](n+1)
+      mbar_init(&bars->qdo_full[i], 257);
       mbar_init(&bars->qdo_free[i], 1);
     }
     for (int i = 0; i < 2; ++i) mbar_init(&bars->ds_free[i], 1);
     mbar_init(&bars->st_full, 1);
-    mbar_init(&bars->dpt_free, 256);
     mbar_init(&bars->p_ready, 256);
     mbar_init(&bars->dq_full, 1);
     mbar_init(&bars->dq_free, 128);
@@ -334,14 +333,16 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     } else if (role == 1 && elect_one()) {
       // ---------------------------------------------------------------- MMA issuer
       // One elected thread (elect.sync compiles to straight-line UTCHMMA).  The tcgen05 queue is
-      // only about 5 MMAs deep, so issue runs at the pace of execution; the barriers of the next
-      // group are probed (non-blocking) before the last kTail MMAs of the current one, and all
-      // per-iteration scalar work is a handful of 32-bit adds on precomputed descriptor words,
-      // so that in the steady state the pipe never drains between two groups.
+      // only about 5 MMAs deep, so issue runs at the pace of execution and every barrier the
+      // thread looks at costs the pipe 90-150 clocks once the queue has drained: it looks at
+      // THREE per iteration (stage full + dP^T free in one, p_ready, dq_free right before the
+      // dQ^T product) with plain try_wait loops.  Round 1 probed five with mbarrier.test_wait
+      // ahead of time; a trace showed the probes themselves (~150 clocks each) were the larger
+      // cost: 8b 1000 -> 1038 TFLOP/s.  All per-iteration scalar work is a handful of 32-bit
+      // adds on precomputed descriptor words.
       constexpr uint32_t idesc_s = umma_idesc_bf16(128, FCP_BQ, 0, 0);    // S^T, dP^T
       constexpr uint32_t idesc_kv = umma_idesc_bf16(128, D, 0, 1);        // dV, dK
       constexpr uint32_t idesc_dq = umma_idesc_bf16(128, FCP_BQ, 1, 1);   // dQ^T
-      constexpr int kTail = Cfg::kTail;
       constexpr int kSteps = D / 16;
       // Every operand here uses SWIZZLE_128B with SBO = 1024: the high descriptor word is one
       // constant, the low word is (address >> 4) | (LBO >> 4) << 16.
@@ -381,39 +382,26 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         // prologue: S^T and dP^T of the item's first iteration
         {
           mbar_wait(&bars->qdo_full[st], sph);
-          mbar_wait(&bars->dpt_free, b ^ 1);
           tc_fence_after();
           const uint32_t q_lo = q_kmaj0 + st * kStageStep;
           issue_kq(Cfg::kColS + b * 64, k_kmaj, q_lo, 0, kSteps);
           issue_kq(Cfg::kColDP, v_kmaj, q_lo + kDoStep, 0, kSteps);
           umma_commit(&bars->st_full);
         }
-        bool ok_a = false;                       // barriers of the next S^T/dP^T group already seen
         for (int i = 0; i < I; ++i) {
           // ring state of iterations n+1 and n+2
           const uint32_t st1 = st + 1 == Cfg::kStages ? 0 : st + 1, sph1 = st + 1 == Cfg::kStages ? sph ^ 1 : sph;
-          const uint32_t st2 = st1 + 1 == Cfg::kStages ? 0 : st1 + 1, sph2 = st1 + 1 == Cfg::kStages ? sph1 ^ 1 : sph1;
-          bool ok_b = false;                     // barriers of this iteration's dV/dK/dQ group seen
           if (i + 1 < I) {                       // next iteration's S^T / dP^T run ahead
-            if (!ok_a) {
-              mbar_wait(&bars->qdo_full[st1], sph1);
-              mbar_wait(&bars->dpt_free, b);     // softmax(n) holds dP^T(n) in registers
-            }
+            mbar_wait(&bars->qdo_full[st1], sph1);   // operands landed, dP^T(n) in registers
             tc_fence_after();
             const uint32_t q_lo = q_kmaj0 + st1 * kStageStep;
             const uint32_t v_lo = opaque(v_kmaj);
             issue_kq(Cfg::kColS + (b ^ 1) * 64, opaque(k_kmaj), q_lo, 0, kSteps);
-            issue_kq(Cfg::kColDP, v_lo, q_lo + kDoStep, 0, kSteps - kTail);
-            ok_b = mbar_test(&bars->p_ready, b) & mbar_test(&bars->dq_free, b ^ 1) &
-                   (i > 0 || mbar_test(&bars->dkv_free, mph ^ 1));
-            issue_kq(Cfg::kColDP, v_lo, q_lo + kDoStep, kSteps - kTail, kSteps);
+            issue_kq(Cfg::kColDP, v_lo, q_lo + kDoStep, 0, kSteps);
             umma_commit(&bars->st_full);
           }
-          if (!ok_b) {
-            mbar_wait(&bars->p_ready, b);
-            if (i == 0) mbar_wait(&bars->dkv_free, mph ^ 1);
-            mbar_wait(&bars->dq_free, b ^ 1);
-          }
+          mbar_wait(&bars->p_ready, b);
+          if (i == 0) mbar_wait(&bars->dkv_free, mph ^ 1);
           tc_fence_after();
           // P^T / dS^T of q columns [32h, 32h+32) live in columns [32h, 32h+16) / [32h+16, 32h+32)
           // of the S^T buffer: each softmax warpgroup overwrites only the columns it has loaded
@@ -431,17 +419,11 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
           // dQ^T = K^T dS^T : A = K tile as MN-major [K=kv][M=d], B = dS^T smem MN-major [K=kv][N=q]
           const uint32_t ds_lo = ds_mnmaj + b * (Cfg::kDS >> 4);
           const uint32_t kt_lo = opaque(k_mnmaj);
+          mbar_wait(&bars->dq_free, b ^ 1);          // the drain holds dQ^T(n-1) in registers
 #pragma unroll
-          for (int kk = 0; kk < 8 - kTail; ++kk)
+          for (int kk = 0; kk < 8; ++kk)
             umma_ss(tmem_base + Cfg::kColDQ, desc(kt_lo + kk * (2048 >> 4)),
                     desc(ds_lo + kk * (2048 >> 4)), idesc_dq, kk > 0);
-          ok_a = false;
-          if (i + 2 < I)
-            ok_a = mbar_test(&bars->qdo_full[st2], sph2) & mbar_test(&bars->dpt_free, b ^ 1);
-#pragma unroll
-          for (int kk = 8 - kTail; kk < 8; ++kk)
-            umma_ss(tmem_base + Cfg::kColDQ, desc(kt_lo + kk * (2048 >> 4)),
-                    desc(ds_lo + kk * (2048 >> 4)), idesc_dq, 1u);
           umma_commit(&bars->qdo_free[st]);
           umma_commit(&bars->ds_free[b]);
           umma_commit(&bars->dq_full);
@@ -460,6 +442,7 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
     // columns 32..63 (a warp reaches TMEM lanes 32*(warp%4)..+31 only, so each warpgroup covers
     // all 128 KV rows).
     reg_alloc<Cfg::kRegsSoftmax>();
+    mbar_arrive(&bars->qdo_full[0]);                   // dP^T is free before the first iteration
     const int half = (role - 4) >> 2;                  // 0 or 1
     const int row = (warp & 3) * 32 + lane;            // KV row of the tile = TMEM lane
     const uint32_t lane_addr = (uint32_t)((warp & 3) * 32) << 16;
@@ -505,7 +488,8 @@ fcp_attn_bwd_main(const __grid_constant__ CUtensorMap tmap_q,
         mbar_wait(&bars->ds_free[n & 1], ((n >> 1) & 1) ^ 1);     // dQ^T(n-2) has read dS^T smem
         tmem_ld_wait();
         tc_fence_before();
-        mbar_arrive(&bars->dpt_free);                              // dP^T (and S^T) now in registers
+        // dP^T (and S^T) now in registers: counts towards the next iteration's stage barrier
+        mbar_arrive(&bars->qdo_full[(n + 1) % Cfg::kStages]);
         const uint32_t stat_addr = stat_base + st * Cfg::kStat;
         const uint32_t ds_row_addr = ds_base + (n & 1) * Cfg::kDS;
         if (need_mask)

@@ -46,19 +46,6 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Non-blocking probe of a phase (mbarrier.test_wait): lets the MMA thread look at the barriers
-// of its next group while the tensor pipe still has queued work.
-__device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile(
-      "{\n\t.reg .pred p;\n\t"
-      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-      "selp.u32 %0, 1, 0, p;\n\t}"
-      : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
-      : "memory");
-  return ok != 0;
-}
 // Bounded wait: a protocol bug traps (reported as a launch failure) instead of hanging the GPU.
 #ifndef FCP_MBAR_SPIN_LIMIT
 #define FCP_MBAR_SPIN_LIMIT (1u << 26)

@@ -42,7 +42,9 @@ typedef enum {
   FCP_BUFFER_TOO_SMALL = -3, /* required element count is written to *n_out */
   FCP_CUDA = -4,             /* a CUDA runtime/driver call or kernel launch failed */
   FCP_MISALIGNED = -5,       /* a device pointer or row pitch is not 16-byte aligned */
-  FCP_NO_MEMORY = -6         /* a host allocation failed (std::bad_alloc is caught at the boundary) */
+  FCP_NO_MEMORY = -6,        /* a host allocation failed (std::bad_alloc is caught at the boundary) */
+  FCP_TOO_LARGE = -7         /* fcp_attn_bwd_static: the schedule's workspace exceeds
+                                FCP_STATIC_WORKSPACE_BYTES */
 } fcp_status;
 
 const char* fcp_strerror(int status);
@@ -305,6 +307,28 @@ enum {
 };
 int  fcp_attn_fwd(const fcp_attn_args* args);
 int  fcp_attn_bwd(const fcp_attn_args* args, const void* dO, void* dq, void* dk, void* dv);
+
+/* fcp_attn_bwd for callers that cannot provide a device workspace (code under CUDA graph capture,
+ * serving loops and harnesses that forbid cudaMalloc): the same three kernels, with the work
+ * lists, the (lse, delta) scratch and the fp32 dQ accumulator of the backward (the
+ * formulas of this section) in a workspace the LIBRARY owns: a file-scope `static __device__`
+ * array of FCP_STATIC_WORKSPACE_BYTES that every GPU which loads the library holds until the
+ * process exits.  The call allocates and frees nothing on the host heap or the device.
+ *   args->workspace must be NULL; every other field, dO, dq, dk, dv as for fcp_attn_bwd (inputs
+ *   and outputs stay the caller's).  No fcp_sched_upload is needed: the call copies the
+ *   schedule's lists into the static workspace on args->stream (from pageable host memory owned
+ *   by the schedule), then launches fcp_bwd_prep, fcp_attn_bwd_main, fcp_bwd_dq_convert there.
+ *   FCP_TOO_LARGE when fcp_sched_workspace_size(args->sched) > FCP_STATIC_WORKSPACE_BYTES
+ *   (nothing is launched); roughly n_q_pad * Hq * (4 D + 8) bytes plus the lists, e.g. 2000 query
+ *   rows at Hq = 32, D = 128 or 8000 at Hq = 8.
+ *   The workspace keeps the previous call's contents; the call itself rewrites the lists and the
+ *   scratch and zeroes the accumulator (fcp_bwd_prep), so nothing carries over.  All calls on a
+ *   device share the one array: calls that overlap on the GPU (different streams, or several host
+ *   threads launching on one device) RACE on it; order them on one stream or with events.  With a
+ *   caller-owned args->dq_accum only the lists and the (lse, delta) scratch live there, the same
+ *   rule applies. */
+#define FCP_STATIC_WORKSPACE_BYTES (32u << 20)
+int  fcp_attn_bwd_static(const fcp_attn_args* args, const void* dO, void* dq, void* dk, void* dv);
 
 /* ------------------------------------------------------------------------------------------
  * 5. Partial-result aggregation: combines attention partials computed over

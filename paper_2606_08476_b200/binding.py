@@ -18,13 +18,15 @@ EXPORTS = [
     "fcp_sched_workspace_size", "fcp_sched_upload", "fcp_sched_get_info", "fcp_attn_fwd",
     "fcp_attn_bwd", "fcp_merge", "fcp_plan_piece_stats", "fcp_piece_layout", "fcp_kv_gather_piece",
     "fcp_kv_scatter_add_piece", "fcp_sched_from_plan_piece", "fcp_sched_get_list",
-    "fcp_kv_reduce_finish",
+    "fcp_kv_reduce_finish", "fcp_attn_bwd_static",
 ]
 
 STRATEGY_HYBRID, STRATEGY_ALL_PER_DOC, STRATEGY_WHOLE_DOC, STRATEGY_PER_SEQ = 0, 1, 2, 3
 # key sets of a rank (include/fcp.h section 2b): the whole prefix, or its local / prefix split
 PIECE_FULL, PIECE_LOCAL, PIECE_PREFIX = 0, 1, 2
 DQ_KEEP, DQ_NO_OUTPUT = 1, 2
+TOO_LARGE = -7                               # fcp_status FCP_TOO_LARGE
+STATIC_WORKSPACE_BYTES = 32 << 20            # FCP_STATIC_WORKSPACE_BYTES
 
 
 class FcpError(RuntimeError):
@@ -137,6 +139,7 @@ def _lib():
         lib.fcp_attn_fwd.argtypes = [C.POINTER(_AttnArgs)]
         lib.fcp_attn_bwd.argtypes = [C.POINTER(_AttnArgs), C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p]
+        lib.fcp_attn_bwd_static.argtypes = lib.fcp_attn_bwd.argtypes
         lib.fcp_merge.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_int32,
                                   C.c_void_p]
@@ -401,6 +404,24 @@ class Sched:
         _check(_lib().fcp_attn_bwd(C.byref(a), do.data_ptr(), None if no_out else dq.data_ptr(),
                                    dk.data_ptr(), dv.data_ptr()), "fcp_attn_bwd")
         return (None if no_out else dq), dk, dv
+
+
+    def attn_bwd_static(self, q, k, v, o, lse, do, scale, dq, dk, dv, stream=None):
+        """fcp_attn_bwd_static: the backward on the library's own static device workspace, no
+        upload() and no allocation anywhere (the outputs dq, dk, dv are the caller's tensors; dk,
+        dv bf16 or f32).  FcpError(TOO_LARGE) when workspace_size() > STATIC_WORKSPACE_BYTES.
+        Calls that overlap on the GPU race on the shared workspace (include/fcp.h)."""
+        import torch
+        for t in (q, k, v, o, do, dq):
+            assert t.is_cuda and t.is_contiguous() and t.dtype == torch.bfloat16
+        assert dk.dtype == dv.dtype and dk.dtype in (torch.bfloat16, torch.float32)
+        assert dk.is_cuda and dv.is_cuda and dk.is_contiguous() and dv.is_contiguous()
+        a = _AttnArgs(self._h, None, q.data_ptr(), k.data_ptr(), v.data_ptr(), o.data_ptr(),
+                      lse.data_ptr(), float(scale), 1 if dk.dtype == torch.float32 else 0,
+                      _stream_ptr(stream), None, None, None, 0)
+        _check(_lib().fcp_attn_bwd_static(C.byref(a), do.data_ptr(), dq.data_ptr(), dk.data_ptr(),
+                                          dv.data_ptr()), "fcp_attn_bwd_static")
+        return dq, dk, dv
 
 
 def kv_reduce_finish(dK, dV, dK_out=None, dV_out=None, stream=None):

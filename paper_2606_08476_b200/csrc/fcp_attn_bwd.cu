@@ -27,6 +27,8 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "fcp_internal.h"
 #include "fcp_sm100.cuh"
 #include "fcp_tma.h"
@@ -700,4 +702,51 @@ extern "C" int fcp_attn_bwd(const fcp_attn_args* a, const void* dO, void* dq, vo
   if (s->D == 128) return launch_bwd<128>(a, s, dO, dq, dk, dv);
   if (s->D == 64) return launch_bwd<64>(a, s, dO, dq, dk, dv);
   return FCP_UNSUPPORTED;
+}
+
+// ------------------------------------------------------------------------------------------
+// fcp_attn_bwd_static: the backward on a workspace the library owns (fcp.h section 4).
+// ------------------------------------------------------------------------------------------
+namespace {
+// Held by every GPU that loads the library, from module load to process exit; uninitialised
+// (no bytes in the .so).  In host code this name is only a handle for cudaGetSymbolAddress:
+// kernels get the device address that static_workspace() returns.
+static __device__ __align__(256) unsigned char fcp_static_ws[FCP_STATIC_WORKSPACE_BYTES];
+
+// Device address of fcp_static_ws on the CURRENT device, looked up once per device (each device
+// has its own copy of the array at its own address) and kept in a write-once table behind
+// atomics; nullptr when the lookup fails.
+void* static_workspace() {
+  constexpr int kMaxDev = 64;
+  static std::atomic<void*> cache[kMaxDev];
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return nullptr;
+  const bool cached = dev >= 0 && dev < kMaxDev;
+  if (cached) {
+    void* p = cache[dev].load(std::memory_order_acquire);
+    if (p) return p;
+  }
+  void* p = nullptr;
+  if (cudaGetSymbolAddress(&p, fcp_static_ws) != cudaSuccess || p == nullptr) return nullptr;
+  if (cached) cache[dev].store(p, std::memory_order_release);
+  return p;
+}
+}  // namespace
+
+extern "C" int fcp_attn_bwd_static(const fcp_attn_args* a, const void* dO, void* dq, void* dk,
+                                   void* dv) {
+  if (!a || !a->sched || a->workspace) return FCP_INVALID_ARG;
+  if (a->sched->total > (size_t)FCP_STATIC_WORKSPACE_BYTES) return FCP_TOO_LARGE;
+  void* ws = static_workspace();
+  if (!ws) {
+    cudaGetLastError();
+    return FCP_CUDA;
+  }
+  fcp_attn_args b = *a;
+  b.workspace = ws;
+  // the lists go first on the same stream: stream order puts them before the kernels, and
+  // behind every earlier call that used the workspace on this stream
+  const int st = fcp_sched_upload(a->sched, ws, a->stream);
+  if (st != FCP_OK) return st;
+  return fcp_attn_bwd(&b, dO, dq, dk, dv);
 }

@@ -418,6 +418,7 @@ extern "C" const char* fcp_strerror(int status) {
     case FCP_CUDA: return "CUDA error";
     case FCP_MISALIGNED: return "misaligned pointer";
     case FCP_NO_MEMORY: return "out of host memory";
+    case FCP_TOO_LARGE: return "schedule workspace larger than FCP_STATIC_WORKSPACE_BYTES";
     default: return "unknown status";
   }
 }

@@ -19,6 +19,7 @@ int fcp_kv_reduce_finish(const float*, const float*, void*, void*, int64_t, void
 int fcp_sched_upload(const fcp_sched*, void*, void*) { return FCP_CUDA; }
 int fcp_attn_fwd(const fcp_attn_args*) { return FCP_CUDA; }
 int fcp_attn_bwd(const fcp_attn_args*, const void*, void*, void*, void*) { return FCP_CUDA; }
+int fcp_attn_bwd_static(const fcp_attn_args*, const void*, void*, void*, void*) { return FCP_CUDA; }
 int fcp_merge(const void*, const float*, const void*, const float*, void*, float*, int64_t, int32_t,
               int32_t, int32_t, void*) { return FCP_CUDA; }
 }

@@ -59,7 +59,7 @@ def test_static_workspace_backward_matches_existing_path(fcp, torch):
         assert sched.workspace is None
         assert torch.cuda.memory_allocated() == held_before
         if i >= 2:          # every kernel variant of this call has been loaded by an earlier one
-            assert torch.cuda.mem_get_info()[0] == free_before, "the call took device memory"
+            assert torch.cuda.mem_get_info()[0] >= free_before, "the call took device memory"
         tag = "call %d" % i
         assert torch.equal(dk, g["dk"]), tag + ": dk differs from fcp_attn_bwd"
         assert torch.equal(dv, g["dv"]), tag + ": dv differs from fcp_attn_bwd"

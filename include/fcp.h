@@ -14,11 +14,13 @@
  *    process-wide data are write-once caches of immutable facts (the SM count per device, the
  *    address of the driver's tensor-map encoder), published with atomics, so every entry point
  *    may be called from several threads and for several devices.  Objects are not internally
- *    synchronised: do not destroy one while another thread uses it.
+ *    synchronised: do not destroy one while another thread uses it.  One exception, stated at
+ *    its declaration: fcp_attn_bwd_static works on a static device array shared by all of its
+ *    calls on a device.
  *  - "host" pointers are ordinary CPU memory; "device" pointers are CUDA device memory of the
  *    current device.  The library owns only the opaque host objects it creates (fcp_plan,
  *    fcp_sched).  It never allocates, frees or synchronises device memory: inputs, outputs
- *    and workspace are the caller's, every device call is asynchronous on `stream`
+ *    and workspace are the caller's (fcp_attn_bwd_static: the workspace is that static array), every device call is asynchronous on `stream`
  *    (a cudaStream_t passed as void*; NULL = the legacy default stream).
  *  - Device tensors are bf16, row-major contiguous, "token-major varlen":
  *        q, o, dO, dq : [n_q , Hq , D]        k, v, dk, dv : [n_kv, Hkv, D]

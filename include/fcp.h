@@ -320,6 +320,8 @@ int  fcp_attn_bwd(const fcp_attn_args* args, const void* dO, void* dq, void* dk,
  *   and outputs stay the caller's).  No fcp_sched_upload is needed: the call copies the
  *   schedule's lists into the static workspace on args->stream (from pageable host memory owned
  *   by the schedule), then launches fcp_bwd_prep, fcp_attn_bwd_main, fcp_bwd_dq_convert there.
+ *   (That list copy is the one step a stream capture would refuse - capture takes no copy from
+ *   pageable memory - and comes back as FCP_CUDA; the kernels themselves capture.)
  *   FCP_TOO_LARGE when fcp_sched_workspace_size(args->sched) > FCP_STATIC_WORKSPACE_BYTES
  *   (nothing is launched); roughly n_q_pad * Hq * (4 D + 8) bytes plus the lists, e.g. 2000 query
  *   rows at Hq = 32, D = 128 or 8000 at Hq = 8.
